@@ -1,0 +1,204 @@
+"""numpy front end of the CPU oracle (oracle/pic_ref.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference leg may import this package.  It does
+not import, and is not imported by, paper_1603_02886_b200.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+from typing import Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "pic_ref.c")
+_LIB = os.path.join(_HERE, "libpicref.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2, IEEE semantics: no fast-math, no FMA contraction."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".%d.tmp" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fPIC", "-shared",
+                               "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Grid(ctypes.Structure):
+    _fields_ = [("dim", ctypes.c_int32), ("n", ctypes.c_int32 * 3), ("h", ctypes.c_double * 3),
+                ("order", ctypes.c_int32), ("dtype", ctypes.c_int32)]
+
+
+@dataclass(frozen=True)
+class Grid:
+    dim: int
+    n: Tuple[int, ...]
+    h: Tuple[float, ...]
+    order: int
+    dtype: str  # "f32" | "f64"
+
+    @property
+    def cells(self) -> int:
+        return int(np.prod(self.n[: self.dim]))
+
+    @property
+    def np_dtype(self):
+        return np.float64 if self.dtype == "f64" else np.float32
+
+    def c(self) -> _Grid:
+        g = _Grid()
+        g.dim = self.dim
+        for k in range(3):
+            g.n[k] = self.n[k] if k < self.dim else 1
+            g.h[k] = self.h[k] if k < self.dim else 1.0
+        g.order = self.order
+        g.dtype = 1 if self.dtype == "f64" else 0
+        return g
+
+
+def grid_of(cfg) -> Grid:
+    """Grid of a pic_workloads.Config."""
+    return Grid(cfg.dim, tuple(cfg.n), tuple([cfg.h] * cfg.dim), cfg.order, cfg.dtype)
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        lib.pic_ref_bspline.argtypes = [ctypes.c_int, ctypes.c_double]
+        lib.pic_ref_bspline.restype = ctypes.c_double
+        for name in ("pic_ref_stencil_1d", "pic_ref_keys", "pic_ref_sort", "pic_ref_deposit",
+                     "pic_ref_deposit_allpairs", "pic_ref_gather", "pic_ref_gather_allnodes",
+                     "pic_ref_push", "pic_ref_step"):
+            getattr(lib, name).restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def _ptrs(arrs: Sequence[np.ndarray]):
+    p = (ctypes.c_void_p * 3)()
+    for k in range(3):
+        p[k] = arrs[k].ctypes.data if k < len(arrs) else None
+    return p
+
+
+def _chk(g: Grid, arrs, n=None, dtype=None):
+    dt = dtype or g.np_dtype
+    for a in arrs:
+        assert isinstance(a, np.ndarray) and a.dtype == dt and a.flags.c_contiguous, (a.dtype, dt)
+        if n is not None:
+            assert a.shape == (n,), (a.shape, n)
+
+
+def _rc(rc):
+    if rc != 0:
+        raise ValueError("oracle: bad argument (rc=%d)" % rc)
+
+
+def bspline(p: int, t: float) -> float:
+    return _load().pic_ref_bspline(int(p), float(t))
+
+
+def stencil_1d(g: Grid, c: int, x: np.ndarray, i: int = 0):
+    """(node indices, weights) of particle i in dimension c."""
+    _chk(g, [x])
+    idx = np.zeros(4, np.int32)
+    wt = np.zeros(4, np.float64)
+    cg = g.c()
+    m = _load().pic_ref_stencil_1d(ctypes.byref(cg), c, ctypes.c_void_p(x.ctypes.data),
+                                   ctypes.c_int64(i), ctypes.c_void_p(idx.ctypes.data),
+                                   ctypes.c_void_p(wt.ctypes.data))
+    if m < 0:
+        _rc(m)
+    return idx[:m].copy(), wt[:m].copy()
+
+
+def keys(g: Grid, x) -> np.ndarray:
+    n = x[0].shape[0]
+    _chk(g, x, n)
+    key = np.empty(n, np.int32)
+    cg = g.c()
+    _rc(_load().pic_ref_keys(ctypes.byref(cg), ctypes.c_int64(n), _ptrs(x),
+                             ctypes.c_void_p(key.ctypes.data)))
+    return key
+
+
+def sort(g: Grid, x, v, w):
+    """-> (x_out, v_out, w_out, perm[n] int32, cell_offsets[C+1] int32)."""
+    n = w.shape[0]
+    _chk(g, list(x) + list(v) + [w], n)
+    xo = [np.empty_like(a) for a in x]
+    vo = [np.empty_like(a) for a in v]
+    wo = np.empty_like(w)
+    perm = np.empty(n, np.int32)
+    off = np.empty(g.cells + 1, np.int32)
+    cg = g.c()
+    _rc(_load().pic_ref_sort(ctypes.byref(cg), ctypes.c_int64(n), _ptrs(x), _ptrs(v),
+                             ctypes.c_void_p(w.ctypes.data), _ptrs(xo), _ptrs(vo),
+                             ctypes.c_void_p(wo.ctypes.data), ctypes.c_void_p(perm.ctypes.data),
+                             ctypes.c_void_p(off.ctypes.data)))
+    return xo, vo, wo, perm, off
+
+
+def deposit(g: Grid, x, w, allpairs: bool = False) -> np.ndarray:
+    """rho[C] in float64, x fastest."""
+    n = w.shape[0]
+    _chk(g, list(x) + [w], n)
+    rho = np.empty(g.cells, np.float64)
+    cg = g.c()
+    f = _load().pic_ref_deposit_allpairs if allpairs else _load().pic_ref_deposit
+    _rc(f(ctypes.byref(cg), ctypes.c_int64(n), _ptrs(x), ctypes.c_void_p(w.ctypes.data),
+          ctypes.c_void_p(rho.ctypes.data)))
+    return rho
+
+
+def gather(g: Grid, x, E, allnodes: bool = False):
+    """Field at the particles, float64, one array per dimension."""
+    n = x[0].shape[0]
+    _chk(g, x, n)
+    _chk(g, E, g.cells)
+    Ep = [np.empty(n, np.float64) for _ in range(g.dim)]
+    cg = g.c()
+    f = _load().pic_ref_gather_allnodes if allnodes else _load().pic_ref_gather
+    _rc(f(ctypes.byref(cg), ctypes.c_int64(n), _ptrs(x), _ptrs(E), _ptrs(Ep)))
+    return Ep
+
+
+def push(g: Grid, x, v, E, dt: float, qm: float):
+    """accel + push; returns new (x, v) (inputs are not modified)."""
+    n = x[0].shape[0]
+    _chk(g, list(x) + list(v), n)
+    _chk(g, E, g.cells)
+    xo = [a.copy() for a in x]
+    vo = [a.copy() for a in v]
+    cg = g.c()
+    _rc(_load().pic_ref_push(ctypes.byref(cg), ctypes.c_int64(n), _ptrs(xo), _ptrs(vo), _ptrs(E),
+                             ctypes.c_double(dt), ctypes.c_double(qm)))
+    return xo, vo
+
+
+def step(g: Grid, x, v, w, E, dt: float, qm: float, do_sort: bool = True, cell_offsets=None):
+    """sort -> deposit(x^t) -> accel -> push.  -> dict(x, v, w, perm, cell_offsets, rho)."""
+    n = w.shape[0]
+    _chk(g, list(x) + list(v) + [w], n)
+    _chk(g, E, g.cells)
+    xo = [np.empty_like(a) for a in x]
+    vo = [np.empty_like(a) for a in v]
+    wo = np.empty_like(w)
+    perm = np.empty(n, np.int32)
+    off = np.empty(g.cells + 1, np.int32) if cell_offsets is None else cell_offsets.copy()
+    rho = np.empty(g.cells, np.float64)
+    cg = g.c()
+    _rc(_load().pic_ref_step(ctypes.byref(cg), ctypes.c_int64(n), _ptrs(x), _ptrs(v),
+                             ctypes.c_void_p(w.ctypes.data), _ptrs(xo), _ptrs(vo),
+                             ctypes.c_void_p(wo.ctypes.data), ctypes.c_void_p(perm.ctypes.data),
+                             ctypes.c_void_p(off.ctypes.data), ctypes.c_void_p(rho.ctypes.data),
+                             _ptrs(E), ctypes.c_double(dt), ctypes.c_double(qm),
+                             ctypes.c_int(1 if do_sort else 0)))
+    return dict(x=xo, v=vo, w=wo, perm=perm, cell_offsets=off, rho=rho)
