@@ -1,0 +1,376 @@
+#!/usr/bin/env python
+"""bench.py -- particle-steps/s of the fused hot path (sort + deposit + push) on B200.
+
+Contract (one JSON line on stdout, rank 0):
+  python bench.py --gpus N --steps K --warmup W [--config cfg3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (pic_step: cell keys, histogram, prefix sum, stable
+scatter, reorder, B-spline deposit, gather + accel + push) over all N_p particles of the workload.
+Default workload: BASELINE.json configs[2] (3-D 128^3, 1e8 particles, fp32, cubic), the
+configuration the metric is quoted on.  The simulation runs continuously from the seeded, unsorted
+initial condition: the W warm-up steps include the first (random-order) sort; the K timed steps are
+the steady state ("10 steps, sort every step").  The first-step time is reported separately.
+
+N > 1 (torchrun): the path does not shard (north_star: one GPU, no collectives) -- "replicas only":
+every rank runs an independent replica with its own seed; value = all particle-steps / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "particle-steps/s (sort+deposit+push)"
+UNIT = "particle-steps/s"
+
+
+def algorithmic_bytes(cfg):
+    """compulsory bytes per particle-step (integer side arrays are overhead)."""
+    d, s = cfg.dim, (8 if cfg.dtype == "f64" else 4)
+    A = 2 * d + 1
+    return {
+        "step": (9 * d + 3) * s,            # sort (d + 2A) + one pass reading A, writing 2d
+        "nosort_step": (4 * d + 1) * s,
+        "keys": d * s,
+        "reorder": 2 * A * s,
+        "deposit": (d + 1) * s,
+        "push": 4 * d * s,
+        "fused": (4 * d + 1) * s,
+    }
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(cfg_name, kernel):
+    """dram bytes read+written per launch of the dominant kernel, from the committed ncu capture
+    (profiles/ncu_traffic.json, written by hand from `ncu --set full`); None if not captured."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    try:
+        return json.load(open(p)).get("%s:%s" % (cfg_name, kernel))
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for k, nme in enumerate(names):
+                    if r[3 + k].strip().lower() == "active":
+                        reasons.add(nme)
+            except Exception:
+                continue
+        if sm:
+            out = {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                   "samples": len(sm)}
+        return out
+
+
+def run_reference(args, cfg_full):
+    """--impl reference: the CPU oracle as it stands, on the box's host cores, bounded sample."""
+    import oracle as O
+    import pic_workloads as W
+    sample = min(cfg_full.N, args.ref_particles)
+    cfg = cfg_full.scaled(sample)
+    wl = W.make_workload(cfg)
+    g = O.grid_of(cfg)
+    x, v, w = wl.x, wl.v, wl.w
+    for _ in range(args.warmup):
+        r = O.step(g, x, v, w, wl.E, cfg.dt, cfg.qm)
+        x, v, w = r["x"], r["v"], r["w"]
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        r = O.step(g, x, v, w, wl.E, cfg.dt, cfg.qm)
+        x, v, w = r["x"], r["v"], r["w"]
+    el = time.perf_counter() - t0
+    val = sample * args.steps / el
+    desc = "first %d particles of %s on the full %s grid, %d steps (sort every step)" % (
+        sample, cfg_full.name, "x".join(map(str, cfg.n)), args.steps)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype,
+            "data": "synthetic", "config": workload_config(cfg_full, args, sample=sample),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(cfg, args, sample=None):
+    return {"workload": "%s: %dD periodic %s grid, %.3g particles, %s, B-spline order %d, %s, sort every %d step(s)" % (
+                cfg.name, cfg.dim, "x".join(map(str, cfg.n)), cfg.N, cfg.dtype, cfg.order,
+                "clustered" if cfg.clustered else "uniform", cfg.sort_every),
+            "particles": cfg.N if sample is None else sample, "grid": list(cfg.n), "order": cfg.order,
+            "sort_every": cfg.sort_every, "parallelism": "replicas" if args.gpus > 1 else "single",
+            "l2": "inputs larger than L2 (no flush needed)" if cfg.N * (2 * cfg.dim + 1) * (8 if cfg.dtype == "f64" else 4) > 256e6
+                  else "working set fits L2; rho/ws rewritten between steps",
+            "timed": "steady state after warm-up steps that include the first random-order sort"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg3")
+    ap.add_argument("--particles", type=int, default=0, help="override N (debug; invalidates the headline)")
+    ap.add_argument("--sort-every", type=int, default=0)
+    ap.add_argument("--ppc", type=int, default=0, help="config 5: particles per cell")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-particles", type=int, default=2_000_000)
+    ap.add_argument("--cpu-particles", type=int, default=10_000_000)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    import pic_workloads as W
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    cfg = W.CONFIGS[args.config]
+    if args.config == "cfg5":
+        cfg = W.cfg5(args.ppc or 128, args.sort_every or 1)
+    if args.particles:
+        cfg = cfg.scaled(args.particles)
+    if args.sort_every:
+        cfg = cfg.scaled(cfg.N, sort_every=args.sort_every)
+
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, cfg)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_1603_02886_b200 as B
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cfg_rank = cfg.scaled(cfg.N, seed=cfg.seed + rank)          # replicas only: independent seeds
+    g = B.grid_of(cfg_rank)
+    wl = W.make_workload(cfg_rank)
+    st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, device=dev)
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up: includes the first, random-order step (timed separately)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    step_no = 0
+    first_ms = None
+    for k in range(args.warmup):
+        e0.record()
+        st.step(cfg.dt, cfg.qm, do_sort=(step_no % cfg.sort_every == 0))
+        e1.record()
+        torch.cuda.synchronize()
+        if k == 0:
+            first_ms = e0.elapsed_time(e1)
+        step_no += 1
+
+    # ---- timed region: exactly K steps, device-timed, with per-phase events
+    K = args.steps
+    phase_ev = [[torch.cuda.Event(enable_timing=True) for _ in B.PHASES] for _ in range(K)]
+    for evs in phase_ev:
+        for e in evs:
+            e.record()
+    launches = 0
+    sorts = 0
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_begin.record()
+    for k in range(K):
+        do_sort = (step_no % cfg.sort_every == 0)
+        B.pic_set_phase_events(phase_ev[k])
+        st.step(cfg.dt, cfg.qm, do_sort=do_sort)
+        launches += B.pic_last_launch_count()
+        sorts += int(do_sort)
+        step_no += 1
+    t_end.record()
+    B.pic_set_phase_events(None)
+    barrier()
+    clocks = sampler.stop()
+    ms_total = t_begin.elapsed_time(t_end)
+    if world > 1:
+        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / K
+    value = cfg.N * world * K / (ms_total * 1e-3)
+
+    # ---- per-phase durations from the events recorded inside the timed region
+    phases = {}
+    for k in range(K):
+        evs, prev = phase_ev[k], phase_ev[k][0]
+        for name, e in list(zip(B.PHASES, evs))[1:]:
+            try:
+                dt_ms = prev.elapsed_time(e)
+            except Exception:
+                continue
+            if dt_ms > 0:
+                phases.setdefault(name, []).append(dt_ms)
+                prev = e
+    phase_ms = {k: sum(v) / len(v) for k, v in phases.items() if v}
+
+    peak, peak_src = measured_peaks()
+    ab = algorithmic_bytes(cfg)
+    dom = max(phase_ms, key=phase_ms.get) if phase_ms else None
+    kernel_bytes = {"keys": ab["keys"], "scan": 0, "radix": 0, "reorder": ab["reorder"], "deposit": ab["deposit"],
+                    "push": ab["push"]}
+    roofline = None
+    if dom:
+        bpp = kernel_bytes.get(dom, 0)
+        if B.FUSED_PHASE_IS_PUSH and dom == "push":
+            bpp = B.fused_kernel_bytes(cfg.dim, 8 if cfg.dtype == "f64" else 4, sorts > 0)
+        ach = bpp * cfg.N / (phase_ms[dom] * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
+                    "frac": ach / peak, "traffic": ncu_traffic(cfg.name, dom),
+                    "peak_source": peak_src, "algorithmic_bytes_per_particle": bpp,
+                    "kernel_ms": phase_ms[dom]}
+    bytes_step = ab["step"] if cfg.sort_every == 1 else (ab["step"] * sorts + ab["nosort_step"] * (K - sorts)) / K
+    step_ach = bytes_step * cfg.N / (ms_step * 1e-3) / 1e9
+
+    # ---- end to end through the host-buffer entry point (pinned host memory, copies timed)
+    e2e = None
+    if not args.no_e2e:
+        e2e = run_e2e(B, torch, cfg_rank, g, wl, dev, K, world, dist if world > 1 else None)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    cpu_baseline = None
+    if not args.no_cpu_baseline and world == 1:
+        cpu_baseline = run_cpu_baseline(cfg, args.cpu_particles)
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": cfg.dtype, "data": "synthetic", "config": workload_config(cfg, args),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+            "cpu_baseline": cpu_baseline,
+            "step_roofline": {"bytes_per_particle_step": bytes_step, "achieved": step_ach, "peak": peak,
+                              "frac": step_ach / peak, "frac_of_8TBps_nominal": step_ach / 8000.0, "unit": "GB/s"},
+            "phase_ms": phase_ms, "first_step_ms": first_ms}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_e2e(B, torch, cfg, g, wl, dev, K, world, dist):
+    """Same metric through pic_step_host: every step copies the particles host->device from pinned
+    memory, runs the step, and reads the advanced particles, perm, cell_offsets and rho back."""
+    n, d = cfg.N, cfg.dim
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    A = dict(x=[pin(a) for a in wl.x], v=[pin(a) for a in wl.v], w=pin(wl.w))
+    Bf = dict(x=[torch.empty_like(a).pin_memory() for a in A["x"]],
+              v=[torch.empty_like(a).pin_memory() for a in A["v"]], w=torch.empty_like(A["w"]).pin_memory())
+    E = [pin(a) for a in wl.E]
+    perm = torch.empty(max(n, 4), dtype=torch.int32).pin_memory()
+    off = torch.empty(g.cells + 1, dtype=torch.int32).pin_memory()
+    rho = torch.empty(g.cells, dtype=g.torch_dtype).pin_memory()
+    dws = torch.empty(B.pic_step_host_bytes(g, n), dtype=torch.uint8, device=dev)
+    s = g.itemsize
+    h2d = (2 * d + 1) * s * n + d * s * g.cells
+    d2h = (2 * d + 1) * s * n + 4 * n + 4 * (g.cells + 1) + s * g.cells
+    steps = max(1, min(K, 5))
+    cur, nxt = A, Bf
+    for k in range(2 + steps):
+        if k == 2:
+            if dist is not None:
+                dist.barrier()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+        B.pic_step_host(g, cur["x"], cur["v"], cur["w"], nxt["x"], nxt["v"], nxt["w"], perm, off, rho, E,
+                        cfg.dt, cfg.qm, True, dws)
+        cur, nxt = nxt, cur
+    torch.cuda.synchronize()
+    el = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([el], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        el = float(t.item())
+    return {"value": n * world * steps / el, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+            "steps": steps, "ms_per_step": 1e3 * el / steps,
+            "api": "pic_step_host (pinned host buffers, sort every step)"}
+
+
+def run_cpu_baseline(cfg, sample):
+    """The oracle as it stands (single thread) on a bounded sample of the same workload."""
+    import oracle as O
+    import pic_workloads as W
+    sample = min(sample, cfg.N)
+    c = cfg.scaled(sample)
+    wl = W.make_workload(c)
+    g = O.grid_of(c)
+    t0 = time.perf_counter()
+    O.step(g, wl.x, wl.v, wl.w, wl.E, c.dt, c.qm)
+    el = time.perf_counter() - t0
+    return {"value": sample / el, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "first %d particles of %s on the full grid, 1 step (sort+deposit+push) from the seeded random order, %.1f s"
+                      % (sample, cfg.name, el),
+            "host_cores_available": os.cpu_count()}
+
+
+if __name__ == "__main__":
+    main()

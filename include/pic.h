@@ -1,0 +1,180 @@
+/*
+ * pic.h -- C-ABI boundary of the B200-native particle hot path of PIC_ENGINE
+ * (arXiv 1603.02886): per-step sort by cell key, B-spline charge deposit, field
+ * gather + accel + push.  Implementation: paper_1603_02886_b200/csrc (CUDA, sm_100a).
+ *
+ * Citations are lines of /root/reference/PAPER.md plus the section they fall in;
+ * R<n> are the readings of silent/garbled passages listed in DESIGN.md.
+ *
+ * Conventions common to every entry point
+ * ---------------------------------------
+ *  - Pointers inside pic_particles_t, rho, E[], perm, cell_offsets and ws are DEVICE
+ *    pointers unless an argument says "host".  pic_grid_t / pic_particles_t themselves
+ *    are small host structs passed by pointer and read before the call returns.
+ *  - Particles are a contiguous structure of arrays, one array per attribute
+ *    ("part_att(num_part, natt)", SoA, section 3.1): x[c], v[c] for
+ *    c < dim, and the weight w (R2).  Element type = grid->dtype (float or double).
+ *    Unused components (c >= dim) are ignored and may be NULL.
+ *  - Grid arrays are x fastest: node (jx,jy,jz) at jx + n[0]*(jy + n[1]*jz)
+ *    ("rho[(..)+nx*(..)+nx*ny*iz2]", App. B).  n nodes per dimension,
+ *    periodic, node j at coordinate j*h (R4).  E is three separate grids
+ *    (section 4.2).
+ *  - Ownership: the caller owns every buffer, including the workspace; the library
+ *    allocates nothing, frees nothing and keeps no particle or grid state between calls
+ *    (the only per-thread state is the launch counter and the optional phase-event hook below).
+ *  - Execution: all work is enqueued on `stream` (a cudaStream_t passed as void*);
+ *    no host synchronisation and no host<->device copy happens inside ("data transfers
+ *    ... kept to a minimum").  Results are valid once the stream is synced.
+ *  - Errors: every function returns a pic_status_t.  Arguments are validated on the
+ *    host BEFORE any launch: dim in {2,3}; order in {1,2,3}; n[c] >= order+1 for
+ *    c < dim; prod n < 2^31; h[c] > 0; 0 <= N < 2^30; non-null pointers aligned to 16 bytes (arrays
+ *    of an empty particle set may be NULL); workspace >= pic_workspace_bytes.  A failed launch gives PIC_ERR_CUDA.
+ *  - Precondition, not checked: 0 <= x[c] < n[c]*h[c].  Cell indices are clamped
+ *     and stencil nodes are folded mod n, so out-of-range positions can
+ *    never cause an out-of-bounds access, only a meaningless deposit.
+ */
+#ifndef PIC_H_
+#define PIC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { PIC_F32 = 0, PIC_F64 = 1 } pic_dtype_t;
+
+typedef enum {
+    PIC_OK = 0,
+    PIC_ERR_INVALID_ARG = -1,   /* null/misaligned pointer, bad dim/order/n/h/N */
+    PIC_ERR_UNSUPPORTED = -2,   /* valid request this build has no kernel for */
+    PIC_ERR_WORKSPACE = -3,     /* ws_bytes < pic_workspace_bytes() */
+    PIC_ERR_CUDA = -4           /* launch failure; see cudaGetLastError() */
+} pic_status_t;
+
+/* How the particle array handed to pic_deposit / pic_push is ordered. */
+typedef enum {
+    PIC_ORDER_UNSORTED = 0,     /* arbitrary order: threads-on-particles with global atomics
+                                   (setrho 3.3.4) */
+    PIC_ORDER_SORTED = 1,       /* sorted by cell key and cell_offsets describes it exactly */
+    PIC_ORDER_STALE = 2         /* sorted some steps ago: mostly local, exactness still required */
+} pic_order_t;
+
+typedef struct {
+    int32_t dim;        /* 2 or 3 */
+    int32_t n[3];       /* cells = nodes per dimension; n[2] ignored when dim == 2 */
+    double  h[3];       /* grid spacing; box length L[c] = n[c]*h[c]; origin 0 */
+    int32_t order;      /* B-spline degree p: 1 (the paper's linear splines), 2, 3 (R1) */
+    int32_t dtype;      /* pic_dtype_t of particles, rho and E */
+} pic_grid_t;
+
+typedef struct {
+    void   *x[3];       /* positions  x[c][N], device */
+    void   *v[3];       /* velocities v[c][N], device */
+    void   *w;          /* weights    w[N],    device */
+    int64_t n;          /* number of particles N */
+} pic_particles_t;
+
+/* Bytes of device workspace that pic_sort / pic_deposit / pic_step need for N particles
+ * on this grid (a multiple of 256).  Pure host computation. */
+int pic_workspace_bytes(const pic_grid_t *grid, int64_t n, size_t *bytes /* host, out */);
+
+/*
+ * pic_sort -- stable counting sort of the particles by cell key (rows a1-a4).
+ *   key_i = c_x + n_x*(c_y + n_y*c_z), c = clamp(floor(x/h), 0, n-1): the particle's target
+ *   bucket, one cell per bucket, bins x fastest (section 3.2; 489-497 App. B).
+ *   histogram -> exclusive prefix sum -> scatter (Alg. 2 lines 1-5).
+ *   The paper's atomic-counter scatter leaves the order inside a bucket arbitrary; here ties keep
+ *   ascending source index, so perm is unique (R7).  floor(x/h) is an IEEE division in the storage
+ *   dtype (R13).
+ * in  : particles in any order (read only).
+ * out : the same particles grouped by cell, out_a[j] = in_a[perm[j]] bit for bit.  Out of place
+ *       (PAPER.md:120-122); `out` must not alias `in` -- the caller ping-pongs instead of the
+ *       paper's copy-back.
+ * perm[N]          : int32, perm[j] = source index of the particle now at position j (R9).
+ * cell_offsets[C+1]: int32, particles of cell k occupy [cell_offsets[k], cell_offsets[k+1]).
+ */
+int pic_sort(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t *out,
+             int32_t *perm, int32_t *cell_offsets, void *ws, size_t ws_bytes, void *stream);
+
+/*
+ * pic_deposit -- charge deposition, setrho (row a5; PAPER.md:79 step i, 200, 292-294 section 3.3.4,
+ * CUDA kernel PAPER.md:479-526).
+ *   rho[j] = h^-d * sum_i w_i * prod_c W_p(x_ic/h_c - j_c), (p+1)^d nodes per particle, periodic.
+ *   p = 1 reproduces the paper's 8 trilinear products; w and 1/h^d are R2.
+ * rho[C] is OVERWRITTEN (R10).  Summation order is unspecified (atomics): results agree with
+ * the oracle to rounding, not bit for bit.
+ * order/cell_offsets: PIC_ORDER_SORTED selects the per-block tile path (shared-memory two-stage
+ * reduction, "sorting is required"); cell_offsets may be NULL for UNSORTED.
+ */
+int pic_deposit(const pic_grid_t *grid, const pic_particles_t *p, int order_state,
+                const int32_t *cell_offsets, void *rho, void *ws, size_t ws_bytes, void *stream);
+
+/*
+ * pic_push -- field gather + accel + push in one pass (rows a6-a7; PAPER.md:82-83 steps iii-iv,
+ * 86, 88; models PAPER.md:312, 316):
+ *   E_i = sum_j E[j] * prod_c W_p(x_ic/h_c - j_c)   (same splines as the deposit)
+ *   v_i += qm*dt*E_i          (field at the OLD position)
+ *   x_i += dt*v_i             (the NEW velocity), then x -= L*floor(x/L); 0 <= x < L in storage.
+ * x and v are updated in place; w is not read.  E[c][C] for c < dim, each a separate grid.
+ */
+int pic_push(const pic_grid_t *grid, pic_particles_t *p, int order_state,
+             const int32_t *cell_offsets, const void *const E[3], double dt, double qm,
+             void *stream);
+
+/*
+ * pic_step -- one time step of the hot path (row a8): sort (if do_sort) -> deposit at x(t) ->
+ * accel -> push, the paper's loop order setrho -> accel -> push with the
+ * field solve left out as in the paper and the re-sort of PAPER.md:100 placed first (R6).
+ * out receives the particles in sorted order, advanced to t+1; rho is the density at t.
+ * do_sort = 0: particles keep their order (out_a[j] = advanced in_a[j]); perm is not written and
+ * cell_offsets (which may be stale or NULL) is not modified.
+ */
+int pic_step(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t *out,
+             int32_t *perm, int32_t *cell_offsets, void *rho, const void *const E[3],
+             double dt, double qm, int do_sort, void *ws, size_t ws_bytes, void *stream);
+
+/*
+ * pic_step_host -- the same step on HOST buffers: copies `in`, E to the device, runs pic_step,
+ * copies out, perm, cell_offsets, rho back and synchronises.  All pointers (including those
+ * inside in/out) are host pointers; dev_ws is a DEVICE scratch buffer of at least
+ * pic_step_host_bytes() bytes.  This is the end-to-end entry bench.py times ("e2e").
+ */
+int pic_step_host_bytes(const pic_grid_t *grid, int64_t n, size_t *bytes /* host, out */);
+int pic_step_host(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t *out,
+                  int32_t *perm, int32_t *cell_offsets, void *rho, const void *const E[3],
+                  double dt, double qm, int do_sort, void *dev_ws, size_t dev_ws_bytes,
+                  void *stream);
+
+/* Number of kernels the last call of this thread enqueued (for bench.py's gpu_launches). */
+int pic_last_launch_count(void);
+
+/*
+ * pic_set_phase_events -- optional per-phase timing.  `events` is a host array of `count`
+ * cudaEvent_t handles (as void*) owned by the caller, or NULL/0 to switch the hook off.  While
+ * set (per host thread), pic_sort / pic_deposit / pic_push / pic_step record events[k] on the
+ * call's stream at the END of phase k (slots >= count are skipped):
+ *   PIC_PHASE_BEGIN 0  before the first kernel      PIC_PHASE_KEYS   1  cell keys + histogram
+ *   PIC_PHASE_SCAN  2  prefix sums                   PIC_PHASE_RADIX  3  stable scatter of (key,index)
+ *   PIC_PHASE_REORDER 4 attribute reorder            PIC_PHASE_DEPOSIT 5 deposit
+ *   PIC_PHASE_PUSH  6  gather + accel + push (or the fused deposit+push kernel)
+ * Recording an event costs no synchronisation; bench.py uses this to time the dominant kernel.
+ */
+#define PIC_PHASE_BEGIN 0
+#define PIC_PHASE_KEYS 1
+#define PIC_PHASE_SCAN 2
+#define PIC_PHASE_RADIX 3
+#define PIC_PHASE_REORDER 4
+#define PIC_PHASE_DEPOSIT 5
+#define PIC_PHASE_PUSH 6
+#define PIC_NUM_PHASES 7
+int pic_set_phase_events(void *const *events /* host */, int count);
+
+/* Static, human-readable text for a pic_status_t. */
+const char *pic_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIC_H_ */

@@ -1,0 +1,174 @@
+// pic_common.cuh -- device-side helpers shared by the kernels of the CUDA path.
+// Nothing here is shared with oracle/ (the CPU oracle has its own statement of everything).
+//
+// Citations: PAPER.md:NNN = line of /root/reference/PAPER.md; R<n> = DESIGN.md reading.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/pic.h"
+
+namespace pic {
+
+constexpr int kMaxPasses = 4;      // radix passes of 8 bits cover 32-bit keys
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+
+// Grid parameters in the storage precision T, passed to kernels by value.
+template <typename T>
+struct GridP {
+    int n[3];        // nodes per dimension (n[2] = 1 in 2-D)
+    T h[3];          // spacing
+    T inv_h[3];      // 1/h (exact when h is a power of two)
+    T L[3];          // box length n*h
+    T inv_L[3];
+    T inv_vol;       // 1 / prod h
+    int hmul;        // 1: every h is a power of two, x*inv_h == x/h bit for bit
+};
+
+template <typename T>
+inline GridP<T> make_gridp(const pic_grid_t& g)
+{
+    GridP<T> p;
+    double vol = 1.0;
+    int hmul = 1;
+    for (int c = 0; c < 3; ++c) {
+        bool on = c < g.dim;
+        p.n[c] = on ? g.n[c] : 1;
+        double h = on ? g.h[c] : 1.0;
+        p.h[c] = (T)h;
+        p.inv_h[c] = (T)1 / p.h[c];
+        double L = (double)p.n[c] * h;
+        p.L[c] = (T)L;
+        p.inv_L[c] = (T)(1.0 / L);
+        if (on) {
+            vol *= h;
+            int e;
+            double m = frexp((double)p.h[c], &e);
+            if (m != 0.5) hmul = 0;
+        }
+    }
+    p.inv_vol = (T)(1.0 / vol);
+    p.hmul = hmul;
+    return p;
+}
+
+// Particle arrays by value (device pointers).
+template <typename T>
+struct PartP {
+    T* x[3];
+    T* v[3];
+    T* w;
+};
+
+template <typename T>
+inline PartP<T> make_partp(const pic_particles_t& p)
+{
+    PartP<T> q;
+    for (int c = 0; c < 3; ++c) { q.x[c] = (T*)p.x[c]; q.v[c] = (T*)p.v[c]; }
+    q.w = (T*)p.w;
+    return q;
+}
+
+// t = x/h by IEEE division in the storage precision (R13); the paper works in grid units,
+// "ix = (int) x".  When h is a power of two the product is the same number.
+template <typename T>
+__device__ __forceinline__ T grid_coord(T x, T h, T inv_h, int hmul)
+{
+    return hmul ? x * inv_h : x / h;
+}
+
+// Clamped cell index: "if (ix<0) ix=0; if (ix>nx-1) ix=nx-1".
+template <typename T>
+__device__ __forceinline__ int cell_index(T t, int n)
+{
+    T f = floor(t);
+    int i = (f < (T)0) ? 0 : ((f > (T)(n - 1)) ? n - 1 : (int)f);
+    return i;
+}
+
+// One-dimensional stencil of degree P: first (unfolded) node and the P+1 weights.
+// xi = t - i0 in [0,1].  P = 1: (1-xi, xi), the factors of PAPER.md:509-519.
+template <typename T, int P>
+__device__ __forceinline__ void spline_weights(T t, int i0, int& first, T (&w)[P + 1])
+{
+    T xi = t - (T)i0;
+    if (P == 1) {
+        first = i0;
+        w[0] = (T)1 - xi;
+        w[1] = xi;
+    } else if (P == 2) {
+        int up = xi >= (T)0.5 ? 1 : 0;
+        T d = xi - (T)up;
+        first = i0 + up - 1;
+        T a = (T)0.5 - d, b = (T)0.5 + d;
+        w[0] = (T)0.5 * a * a;
+        w[1] = (T)0.75 - d * d;
+        w[P] = (T)0.5 * b * b;
+    } else {
+        T om = (T)1 - xi;
+        T x2 = xi * xi;
+        first = i0 - 1;
+        w[0] = om * om * om * (T)(1.0 / 6.0);
+        w[P] = x2 * xi * (T)(1.0 / 6.0);
+        w[1] = (T)(2.0 / 3.0) - x2 + (T)0.5 * x2 * xi;
+        w[P - 1] = (T)(1.0 / 6.0) + (T)0.5 * (xi + x2 - x2 * xi);
+    }
+}
+
+// fold an index in [-n, 2n) into [0, n)
+__device__ __forceinline__ int fold(int j, int n)
+{
+    j = j < 0 ? j + n : j;
+    return j >= n ? j - n : j;
+}
+
+// Periodic wrap of a pushed position into [0, L) in the storage precision.
+template <typename T>
+__device__ __forceinline__ T wrap_periodic(T x, T L, T inv_L)
+{
+    if (x < (T)0 || x >= L) {
+        x -= L * floor(x * inv_L);
+        if (x < (T)0) x += L;
+        if (x >= L) x -= L;
+        if (!(x >= (T)0 && x < L)) x = (T)0;
+    }
+    return x;
+}
+
+#define PIC_CUDA_OK(expr)                          \
+    do {                                           \
+        if ((expr) != cudaSuccess) return PIC_ERR_CUDA; \
+    } while (0)
+
+// thread-local launch counter behind pic_last_launch_count()
+void count_launch(int n = 1);
+// records the caller's event for `phase` on `st` if pic_set_phase_events() installed one
+void mark_phase(int phase, cudaStream_t st);
+
+// ---- launchers implemented in the .cu files (all enqueue on `st`) ------------------------
+struct SortWs {
+    uint32_t* keys[2];
+    uint32_t* idx[2];
+    int32_t* cell_count;     // [C]
+    uint32_t* digit_hist;    // [kMaxPasses][kRadix]
+    uint32_t* scan_status;   // [scan tiles]
+    uint32_t* counters;      // [16]
+    uint32_t* lookback;      // [passes][tiles][kRadix]
+    void* zero_begin;        // region that must be zero before a sort
+    size_t zero_bytes;
+    int passes, bits_per_pass, key_bits;
+    int64_t radix_tiles, scan_tiles;
+};
+
+size_t sort_ws_bytes(const pic_grid_t& g, int64_t n);
+int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, SortWs& out);
+
+int launch_sort(const pic_grid_t& g, const pic_particles_t& in, pic_particles_t& out, int32_t* perm,
+                int32_t* cell_offsets, const SortWs& ws, cudaStream_t st);
+int launch_deposit(const pic_grid_t& g, const pic_particles_t& p, int order_state,
+                   const int32_t* cell_offsets, void* rho, cudaStream_t st);
+int launch_push(const pic_grid_t& g, pic_particles_t& p, int order_state, const int32_t* cell_offsets,
+                const void* const E[3], double dt, double qm, cudaStream_t st);
+
+}  // namespace pic

@@ -1,0 +1,296 @@
+"""GPU parity: the CUDA path, called through the C ABI (include/pic.h), against the CPU oracle on
+the same seeded inputs.  perm and cell_offsets bit-exact; rho, x, v within north_star's tolerances.
+"""
+import numpy as np
+import pytest
+
+import pic_workloads as W
+from parity import TOL_RHO, TOL_XV, err_rho, err_v, err_x, to_dev, to_host
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def _mods():
+    import oracle as O
+    import paper_1603_02886_b200 as B
+    return O, B
+
+
+# sizes span several radix tiles (4096) and scan tiles (2048) plus a ragged tail
+SMALL = [
+    ("cfg1", dict()),                                           # 2-D 64^2, 1e5, f64, p=1 (full size)
+    ("cfg2", dict(N=3 * 4096 + 77)),
+    ("cfg2", dict(N=200_003, n=(64, 64))),
+    ("cfg3", dict(N=150_001, n=(32, 32, 32))),
+    ("cfg3", dict(N=40_000, n=(16, 8, 4))),
+    ("cfg4", dict(N=300_007, n=(32, 32, 32))),
+    ("cfg5", dict(N=8 * 16 ** 3 + 5, n=(16, 16, 16))),
+]
+ORDERS = [1, 2, 3]
+
+
+def _cfg(name, kw, order=None, dtype=None):
+    cfg = W.CONFIGS[name]
+    kw = dict(kw)
+    N = kw.pop("N", cfg.N)
+    cfg = cfg.scaled(N, **kw)
+    if order is not None:
+        cfg = cfg.scaled(N, order=order)
+    if dtype is not None:
+        cfg = cfg.scaled(N, dtype=dtype)
+    return cfg
+
+
+def _gpu_sort(B, g, wl):
+    n = wl.cfg.N
+    x, v = to_dev(wl.x), to_dev(wl.v)
+    w = to_dev([wl.w])[0]
+    xo = [torch.empty_like(a) for a in x]
+    vo = [torch.empty_like(a) for a in v]
+    wo = torch.empty_like(w)
+    perm = torch.full((max(n, 4),), -1, dtype=torch.int32, device="cuda")
+    off = torch.full((g.cells + 4,), -1, dtype=torch.int32, device="cuda")
+    ws = torch.empty(B.pic_workspace_bytes(g, n), dtype=torch.uint8, device="cuda")
+    B.pic_sort(g, x, v, w, xo, vo, wo, perm, off, ws)
+    torch.cuda.synchronize()
+    return xo, vo, wo, perm[:n], off[: g.cells + 1]
+
+
+@pytest.mark.parametrize("name,kw", SMALL)
+def test_sort_bit_exact(name, kw):
+    O, B = _mods()
+    cfg = _cfg(name, kw)
+    wl = W.make_workload(cfg)
+    ro = O.sort(O.grid_of(cfg), wl.x, wl.v, wl.w)
+    xo, vo, wo, perm, off = _gpu_sort(B, B.grid_of(cfg), wl)
+    assert np.array_equal(perm.cpu().numpy(), ro[3])
+    assert np.array_equal(off.cpu().numpy(), ro[4])
+    for c in range(cfg.dim):
+        assert np.array_equal(xo[c].cpu().numpy(), ro[0][c])
+        assert np.array_equal(vo[c].cpu().numpy(), ro[1][c])
+    assert np.array_equal(wo.cpu().numpy(), ro[2])
+    assert B.pic_last_launch_count() >= 5
+
+
+@pytest.mark.parametrize("N", [0, 1, 31, 32, 33, 4095, 4096, 4097, 8192])
+def test_sort_edge_sizes(N):
+    O, B = _mods()
+    cfg = _cfg("cfg2", dict(N=N, n=(16, 16)))
+    wl = W.make_workload(cfg)
+    ro = O.sort(O.grid_of(cfg), wl.x, wl.v, wl.w)
+    xo, vo, wo, perm, off = _gpu_sort(B, B.grid_of(cfg), wl)
+    assert np.array_equal(perm.cpu().numpy(), ro[3])
+    assert np.array_equal(off.cpu().numpy(), ro[4])
+    assert np.array_equal(xo[0].cpu().numpy(), ro[0][0])
+
+
+def test_sort_degenerate_inputs():
+    O, B = _mods()
+    cfg = _cfg("cfg3", dict(N=50_000, n=(16, 16, 16)))
+    wl = W.make_workload(cfg)
+    # (a) every particle in one cell  (b) already sorted  (c) reverse sorted  (d) positions on cell faces and at x = L-ulp
+    one = [np.full(cfg.N, 3.25, np.float32) + (np.arange(cfg.N) % 7).astype(np.float32) * 0.1 for _ in range(3)]
+    for x in (one, None, "rev", "faces"):
+        if x is None:
+            xs, vs, wsrt, _, _ = O.sort(O.grid_of(cfg), wl.x, wl.v, wl.w)
+            wl2 = W.Workload(cfg, xs, vs, wsrt, wl.E, wl.modes)
+        elif isinstance(x, str) and x == "rev":
+            xs, vs, wsrt, _, _ = O.sort(O.grid_of(cfg), wl.x, wl.v, wl.w)
+            wl2 = W.Workload(cfg, [a[::-1].copy() for a in xs], [a[::-1].copy() for a in vs], wsrt[::-1].copy(), wl.E, wl.modes)
+        elif isinstance(x, str):
+            xf = [np.floor(a).astype(np.float32) for a in wl.x]
+            xf[0][::3] = np.nextafter(np.float32(16.0), np.float32(0.0))
+            xf[1][::5] = 0.0
+            wl2 = W.Workload(cfg, xf, wl.v, wl.w, wl.E, wl.modes)
+        else:
+            wl2 = W.Workload(cfg, x, wl.v, wl.w, wl.E, wl.modes)
+        ro = O.sort(O.grid_of(cfg), wl2.x, wl2.v, wl2.w)
+        xo, vo, wo, perm, off = _gpu_sort(B, B.grid_of(cfg), wl2)
+        assert np.array_equal(perm.cpu().numpy(), ro[3])
+        assert np.array_equal(off.cpu().numpy(), ro[4])
+
+
+@pytest.mark.parametrize("order", ORDERS)
+@pytest.mark.parametrize("name,kw", SMALL)
+def test_deposit_parity(name, kw, order):
+    O, B = _mods()
+    cfg = _cfg(name, kw, order=order)
+    wl = W.make_workload(cfg)
+    go, gb = O.grid_of(cfg), B.grid_of(cfg)
+    rho_ref = O.deposit(go, wl.x, wl.w)
+    x, w = to_dev(wl.x), to_dev([wl.w])[0]
+    rho = torch.full((gb.cells,), 123.0, dtype=gb.torch_dtype, device="cuda")      # must be overwritten
+    B.pic_deposit(gb, x, w, rho, B.PIC_ORDER_UNSORTED)
+    assert err_rho(rho.cpu().numpy(), rho_ref) <= TOL_RHO[cfg.dtype]
+    # sorted path
+    xs, vs, wsrt, perm, off = O.sort(go, wl.x, wl.v, wl.w)
+    rho_ref_s = O.deposit(go, xs, wsrt)
+    xd, wd = to_dev(xs), to_dev([wsrt])[0]
+    offd = torch.from_numpy(np.concatenate([off, np.zeros(3, np.int32)])).cuda()
+    ws = torch.empty(B.pic_workspace_bytes(gb, cfg.N), dtype=torch.uint8, device="cuda")
+    rho.fill_(-7.0)
+    B.pic_deposit(gb, xd, wd, rho, B.PIC_ORDER_SORTED, offd, ws)
+    r = rho.cpu().numpy()
+    assert err_rho(r, rho_ref_s) <= TOL_RHO[cfg.dtype]
+    # exact conservation holds at any size: sum rho h^d = sum w
+    tot = float(np.sum(wl.w.astype(np.float64)))
+    assert abs(float(np.sum(r.astype(np.float64))) * cfg.h ** cfg.dim - tot) <= (1e-12 if cfg.dtype == "f64" else 2e-6) * tot
+
+
+@pytest.mark.parametrize("order", ORDERS)
+@pytest.mark.parametrize("name,kw", SMALL)
+def test_push_parity(name, kw, order):
+    O, B = _mods()
+    cfg = _cfg(name, kw, order=order)
+    wl = W.make_workload(cfg)
+    go, gb = O.grid_of(cfg), B.grid_of(cfg)
+    xr, vr = O.push(go, wl.x, wl.v, wl.E, cfg.dt, cfg.qm)
+    x, v, E = to_dev(wl.x), to_dev(wl.v), to_dev(wl.E)
+    B.pic_push(gb, x, v, E, cfg.dt, cfg.qm)
+    for c in range(cfg.dim):
+        xg, vg = x[c].cpu().numpy(), v[c].cpu().numpy()
+        assert err_x(xg, xr[c], cfg.L[c]) <= TOL_XV[cfg.dtype]
+        assert err_v(vg, vr[c]) <= TOL_XV[cfg.dtype]
+        assert np.all((xg >= 0) & (xg < cfg.np_dtype(cfg.L[c])))
+    # sorted input goes through the sorted path
+    xs, vs, wsrt, perm, off = O.sort(go, wl.x, wl.v, wl.w)
+    xr, vr = O.push(go, xs, vs, wl.E, cfg.dt, cfg.qm)
+    x, v = to_dev(xs), to_dev(vs)
+    offd = torch.from_numpy(np.concatenate([off, np.zeros(3, np.int32)])).cuda()
+    B.pic_push(gb, x, v, E, cfg.dt, cfg.qm, B.PIC_ORDER_SORTED, offd)
+    for c in range(cfg.dim):
+        assert err_x(x[c].cpu().numpy(), xr[c], cfg.L[c]) <= TOL_XV[cfg.dtype]
+        assert err_v(v[c].cpu().numpy(), vr[c]) <= TOL_XV[cfg.dtype]
+
+
+def _lockstep(cfg, steps, sort_every=1):
+    """GPU step k is fed the oracle's state after step k-1 (reading R19)."""
+    O, B = _mods()
+    wl = W.make_workload(cfg)
+    go, gb = O.grid_of(cfg), B.grid_of(cfg)
+    x, v, w = wl.x, wl.v, wl.w
+    E = to_dev(wl.E)
+    n = cfg.N
+    ws = torch.empty(B.pic_workspace_bytes(gb, n), dtype=torch.uint8, device="cuda")
+    off_ref = None
+    for k in range(steps):
+        do_sort = (k % sort_every) == 0
+        ref = O.step(go, x, v, w, wl.E, cfg.dt, cfg.qm, do_sort=do_sort, cell_offsets=off_ref)
+        xi, vi, wi = to_dev(x), to_dev(v), to_dev([w])[0]
+        xo = [torch.empty_like(a) for a in xi]
+        vo = [torch.empty_like(a) for a in vi]
+        wo = torch.empty_like(wi)
+        perm = torch.full((max(n, 4),), -1, dtype=torch.int32, device="cuda")
+        if do_sort or off_ref is None:
+            off = torch.full((gb.cells + 4,), -1, dtype=torch.int32, device="cuda")
+        else:
+            off = torch.from_numpy(np.concatenate([off_ref, np.zeros(3, np.int32)])).cuda()
+        rho = torch.empty(gb.cells, dtype=gb.torch_dtype, device="cuda")
+        B.pic_step(gb, xi, vi, wi, xo, vo, wo, perm, off if (do_sort or off_ref is not None) else None, rho, E,
+                   cfg.dt, cfg.qm, do_sort, ws)
+        torch.cuda.synchronize()
+        if do_sort:
+            assert np.array_equal(perm[:n].cpu().numpy(), ref["perm"]), "perm differs at step %d" % k
+            assert np.array_equal(off[: gb.cells + 1].cpu().numpy(), ref["cell_offsets"])
+            off_ref = ref["cell_offsets"]
+        assert err_rho(rho.cpu().numpy(), ref["rho"]) <= TOL_RHO[cfg.dtype], "rho at step %d" % k
+        for c in range(cfg.dim):
+            assert err_x(xo[c].cpu().numpy(), ref["x"][c], cfg.L[c]) <= TOL_XV[cfg.dtype], "x at step %d" % k
+            assert err_v(vo[c].cpu().numpy(), ref["v"][c]) <= TOL_XV[cfg.dtype], "v at step %d" % k
+        assert np.array_equal(wo.cpu().numpy(), ref["w"])
+        x, v, w = ref["x"], ref["v"], ref["w"]
+
+
+@pytest.mark.parametrize("name,kw,steps", [
+    ("cfg1", dict(), 1),
+    ("cfg2", dict(N=300_000, n=(64, 64)), 10),
+    ("cfg3", dict(N=400_000, n=(32, 32, 32)), 10),
+    ("cfg4", dict(N=400_000, n=(32, 32, 32)), 10),
+    ("cfg5", dict(N=32 * 16 ** 3, n=(16, 16, 16)), 6),
+])
+def test_step_lockstep(name, kw, steps):
+    _lockstep(_cfg(name, kw), steps)
+
+
+@pytest.mark.parametrize("k", [4, 16])
+def test_step_lockstep_sort_every_k(k):
+    # config 5's sort-every-k arm: steps between sorts run on the stale order and must stay exact
+    _lockstep(_cfg("cfg5", dict(N=8 * 16 ** 3, n=(16, 16, 16))), 18, sort_every=k)
+
+
+@pytest.mark.parametrize("name,kw", [("cfg2", dict(N=200_000, n=(64, 64))), ("cfg3", dict(N=300_000, n=(32, 32, 32)))])
+def test_step_free_running_by_particle_id(name, kw):
+    """10 steps without re-feeding the oracle state: compare by particle identity (composition of perms)."""
+    O, B = _mods()
+    cfg = _cfg(name, kw)
+    wl = W.make_workload(cfg)
+    go, gb = O.grid_of(cfg), B.grid_of(cfg)
+    st = B.Stepper(gb, wl.x, wl.v, wl.w, wl.E)
+    ident_g = torch.arange(cfg.N, device="cuda")
+    x, v, w = wl.x, wl.v, wl.w
+    ident_r = np.arange(cfg.N)
+    for _ in range(10):
+        st.step(cfg.dt, cfg.qm, True)
+        ident_g = ident_g[st.perm[: cfg.N].long()]
+        r = O.step(go, x, v, w, wl.E, cfg.dt, cfg.qm)
+        ident_r = ident_r[r["perm"]]
+        x, v, w = r["x"], r["v"], r["w"]
+    ig = ident_g.cpu().numpy()
+    inv_g, inv_r = np.empty_like(ig), np.empty_like(ident_r)
+    inv_g[ig] = np.arange(cfg.N)
+    inv_r[ident_r] = np.arange(cfg.N)
+    # a 1-ulp difference can move a particle across a cell face and change later perms; x and v by id must still agree
+    for c in range(cfg.dim):
+        xg = st.cur["x"][c].cpu().numpy()[inv_g]
+        vg = st.cur["v"][c].cpu().numpy()[inv_g]
+        assert err_x(xg, x[c][inv_r], cfg.L[c]) <= 10 * TOL_XV[cfg.dtype]
+        assert err_v(vg, v[c][inv_r]) <= 10 * TOL_XV[cfg.dtype]
+    mism = int(np.sum(ig != ident_r))
+    assert mism <= (0 if cfg.dtype == "f64" else cfg.N // 1000), "order mismatches: %d" % mism
+
+
+def test_step_host_entry_point():
+    O, B = _mods()
+    cfg = _cfg("cfg2", dict(N=50_001, n=(32, 32)))
+    wl = W.make_workload(cfg)
+    go, gb = O.grid_of(cfg), B.grid_of(cfg)
+    ref = O.step(go, wl.x, wl.v, wl.w, wl.E, cfg.dt, cfg.qm)
+    xo = [np.empty_like(a) for a in wl.x]
+    vo = [np.empty_like(a) for a in wl.v]
+    wo = np.empty_like(wl.w)
+    perm = np.empty(cfg.N, np.int32)
+    off = np.empty(gb.cells + 1, np.int32)
+    rho = np.empty(gb.cells, cfg.np_dtype)
+    dws = torch.empty(B.pic_step_host_bytes(gb, cfg.N), dtype=torch.uint8, device="cuda")
+    B.pic_step_host(gb, wl.x, wl.v, wl.w, xo, vo, wo, perm, off, rho, wl.E, cfg.dt, cfg.qm, True, dws)
+    assert np.array_equal(perm, ref["perm"]) and np.array_equal(off, ref["cell_offsets"])
+    assert err_rho(rho, ref["rho"]) <= TOL_RHO[cfg.dtype]
+    for c in range(cfg.dim):
+        assert err_x(xo[c], ref["x"][c], cfg.L[c]) <= TOL_XV[cfg.dtype]
+        assert err_v(vo[c], ref["v"][c]) <= TOL_XV[cfg.dtype]
+
+
+def test_argument_validation():
+    O, B = _mods()
+    g = B.Grid(2, (16, 16), (1.0, 1.0), 1, "f64")
+    n = 100
+    x = [torch.zeros(n, dtype=torch.float64, device="cuda") for _ in range(2)]
+    w = torch.ones(n, dtype=torch.float64, device="cuda")
+    rho = torch.zeros(g.cells, dtype=torch.float64, device="cuda")
+    with pytest.raises(B.PicError):
+        B.pic_deposit(B.Grid(2, (16, 16), (1.0, 1.0), 4, "f64"), x, w, rho)          # order 4
+    with pytest.raises(B.PicError):
+        B.pic_deposit(B.Grid(2, (2, 16), (1.0, 1.0), 3, "f64"), x, w, torch.zeros(32, dtype=torch.float64, device="cuda"))
+    with pytest.raises(B.PicError):
+        B.pic_deposit(B.Grid(2, (16, 16), (0.0, 1.0), 1, "f64"), x, w, rho)          # h = 0
+    ws = torch.empty(16, dtype=torch.uint8, device="cuda")                            # workspace too small
+    perm = torch.empty(n, dtype=torch.int32, device="cuda")
+    off = torch.empty(g.cells + 1, dtype=torch.int32, device="cuda")
+    with pytest.raises(B.PicError, match="workspace"):
+        B.pic_sort(g, x, x, w, [torch.empty_like(a) for a in x], [torch.empty_like(a) for a in x],
+                   torch.empty_like(w), perm, off, ws)
+    ws = torch.empty(B.pic_workspace_bytes(g, n), dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.PicError):                                                   # in aliases out
+        B.pic_sort(g, x, x, w, x, x, w, perm, off, ws)
