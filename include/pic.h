@@ -105,8 +105,12 @@ int pic_sort(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t 
  *   p = 1 reproduces the paper's 8 trilinear products; w and 1/h^d are R2.
  * rho[C] is OVERWRITTEN (R10).  Summation order is unspecified (atomics): results agree with
  * the oracle to rounding, not bit for bit.
- * order/cell_offsets: PIC_ORDER_SORTED selects the per-block tile path (shared-memory two-stage
- * reduction, "sorting is required"); cell_offsets may be NULL for UNSORTED.
+ * order/cell_offsets: PIC_ORDER_SORTED selects the per-cell path (thread-private sums, one global
+ * reduction per node and cell run; "sorting is required");
+ * cell_offsets may be NULL for UNSORTED.
+ * ws: fp32 grids accumulate in a double-precision grid of the workspace (rounded once into rho), so
+ * ws of at least pic_workspace_bytes() is REQUIRED when dtype == PIC_F32; fp64 grids accumulate in
+ * rho itself and ws may be NULL.
  */
 int pic_deposit(const pic_grid_t *grid, const pic_particles_t *p, int order_state,
                 const int32_t *cell_offsets, void *rho, void *ws, size_t ws_bytes, void *stream);

@@ -127,23 +127,28 @@ int pic_sort(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
     if ((rc = carve_sort_ws(*grid, in->n, ws, ws_bytes, sws)) != PIC_OK) return rc;
     pic_particles_t o = *out;
     o.n = in->n;
-    return launch_sort(*grid, *in, o, perm, cell_offsets, sws, (cudaStream_t)stream);
+    return launch_sort(*grid, *in, o, perm, cell_offsets, sws, true, (cudaStream_t)stream);
 }
 
 int pic_deposit(const pic_grid_t* grid, const pic_particles_t* p, int order_state, const int32_t* cell_offsets,
                 void* rho, void* ws, size_t ws_bytes, void* stream)
 {
-    (void)ws;
-    (void)ws_bytes;
     g_launches = 0;
     int rc = check_grid(grid);
     if (rc != PIC_OK) return rc;
     if ((rc = check_particles(*grid, p, false, true)) != PIC_OK) return rc;
+    double* racc = nullptr;
+    if (grid->dtype == PIC_F32) {          // fp32 grids accumulate in a double grid of the workspace
+        if (!aligned16(ws)) return PIC_ERR_INVALID_ARG;
+        SortWs sws;
+        if ((rc = carve_sort_ws(*grid, p->n, ws, ws_bytes, sws)) != PIC_OK) return rc;
+        racc = sws.racc;
+    }
     if (order_state < PIC_ORDER_UNSORTED || order_state > PIC_ORDER_STALE) return PIC_ERR_INVALID_ARG;
     if (order_state != PIC_ORDER_UNSORTED && !aligned16(cell_offsets)) return PIC_ERR_INVALID_ARG;
     if (!aligned16(rho)) return PIC_ERR_INVALID_ARG;
     mark_phase(PIC_PHASE_BEGIN, (cudaStream_t)stream);
-    rc = launch_deposit(*grid, *p, order_state, cell_offsets, rho, (cudaStream_t)stream);
+    rc = launch_deposit(*grid, *p, order_state, cell_offsets, rho, racc, (cudaStream_t)stream);
     mark_phase(PIC_PHASE_DEPOSIT, (cudaStream_t)stream);
     return rc;
 }
@@ -179,12 +184,14 @@ int pic_step(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
     pic_particles_t o = *out;
     o.n = in->n;
     const size_t s = grid->dtype == PIC_F64 ? 8 : 4;
+    if (!aligned16(ws)) return PIC_ERR_INVALID_ARG;
+    SortWs sws;
+    if ((rc = carve_sort_ws(*grid, in->n, ws, ws_bytes, sws)) != PIC_OK) return rc;
     if (do_sort) {
-        if ((in->n > 0 && !aligned16(perm)) || !aligned16(cell_offsets) || !aligned16(ws)) return PIC_ERR_INVALID_ARG;
+        if ((in->n > 0 && !aligned16(perm)) || !aligned16(cell_offsets)) return PIC_ERR_INVALID_ARG;
         if (in->n > 0 && aliases(*grid, *in, *out)) return PIC_ERR_INVALID_ARG;
-        SortWs sws;
-        if ((rc = carve_sort_ws(*grid, in->n, ws, ws_bytes, sws)) != PIC_OK) return rc;
-        if ((rc = launch_sort(*grid, *in, o, perm, cell_offsets, sws, st)) != PIC_OK) return rc;
+        // perm and cell_offsets only: the reorder itself happens inside the fused kernel below
+        if ((rc = launch_sort(*grid, *in, o, perm, cell_offsets, sws, false, st)) != PIC_OK) return rc;
     } else {
         // keep the current order; out may be the same arrays as in (in-place step)
         for (int c = 0; c < grid->dim; ++c) {
@@ -195,7 +202,12 @@ int pic_step(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
     }
     const int order_state = do_sort ? PIC_ORDER_SORTED : (cell_offsets ? PIC_ORDER_STALE : PIC_ORDER_UNSORTED);
     if (!do_sort) mark_phase(PIC_PHASE_BEGIN, st);
-    if ((rc = launch_deposit(*grid, o, order_state, cell_offsets, rho, st)) != PIC_OK) return rc;
+    if (order_state == PIC_ORDER_SORTED) {       // one fused kernel over the sorted particles
+        rc = launch_fused(*grid, *in, o, perm, cell_offsets, rho, E, dt, qm, sws.racc, st);
+        mark_phase(PIC_PHASE_PUSH, st);
+        return rc;
+    }
+    if ((rc = launch_deposit(*grid, o, order_state, cell_offsets, rho, sws.racc, st)) != PIC_OK) return rc;
     mark_phase(PIC_PHASE_DEPOSIT, st);
     rc = launch_push(*grid, o, order_state, cell_offsets, E, dt, qm, st);
     mark_phase(PIC_PHASE_PUSH, st);

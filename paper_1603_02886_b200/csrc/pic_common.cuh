@@ -155,6 +155,7 @@ struct SortWs {
     uint32_t* scan_status;   // [scan tiles]
     uint32_t* counters;      // [16]
     uint32_t* lookback;      // [passes][tiles][kRadix]
+    double* racc;            // [C] double accumulation grid of the deposit (not in the zero region)
     void* zero_begin;        // region that must be zero before a sort
     size_t zero_bytes;
     int passes, bits_per_pass, key_bits;
@@ -164,11 +165,18 @@ struct SortWs {
 size_t sort_ws_bytes(const pic_grid_t& g, int64_t n);
 int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, SortWs& out);
 
+// reorder = false: only perm and cell_offsets are produced (out is not written)
 int launch_sort(const pic_grid_t& g, const pic_particles_t& in, pic_particles_t& out, int32_t* perm,
-                int32_t* cell_offsets, const SortWs& ws, cudaStream_t st);
+                int32_t* cell_offsets, const SortWs& ws, bool reorder, cudaStream_t st);
 int launch_deposit(const pic_grid_t& g, const pic_particles_t& p, int order_state,
-                   const int32_t* cell_offsets, void* rho, cudaStream_t st);
+                   const int32_t* cell_offsets, void* rho, double* racc, cudaStream_t st);
 int launch_push(const pic_grid_t& g, pic_particles_t& p, int order_state, const int32_t* cell_offsets,
                 const void* const E[3], double dt, double qm, cudaStream_t st);
+// deposit at x(t) + gather + accel + push in ONE kernel over particles sorted by cell: in place on
+// p (perm == NULL), or reading particle perm[j] of src and writing slot j of p (the sort's reorder
+// fused into the same pass)
+int launch_fused(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
+                 const int32_t* cell_offsets, void* rho, const void* const E[3], double dt, double qm, double* racc,
+                 cudaStream_t st);
 
 }  // namespace pic

@@ -5,12 +5,13 @@
 // k_deposit_particles is the paper's collision-resolving "threads on particles" algorithm
 // (setrho 3.3.4): one thread per particle, (p+1)^d atomic adds to the grid.
 // It is correct for ANY particle order and is the path for PIC_ORDER_UNSORTED / STALE input.
-#include "pic_common.cuh"
+// Particles sorted by cell (PIC_ORDER_SORTED) go through k_cells (pic_cells.cuh).
+#include "pic_cells.cuh"
 
 namespace pic {
 
 template <typename T, int D, int P>
-__global__ void __launch_bounds__(256) k_deposit_particles(PartP<T> p, GridP<T> g, int64_t n, T* __restrict__ rho)
+__global__ void __launch_bounds__(256) k_deposit_particles(PartP<T> p, GridP<T> g, int64_t n, double* __restrict__ rho)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -30,7 +31,7 @@ __global__ void __launch_bounds__(256) k_deposit_particles(PartP<T> p, GridP<T> 
 #pragma unroll
             for (int a = 0; a <= P; ++a) {
                 const int jx = fold(first[0] + a, g.n[0]);
-                atomicAdd(&rho[jx + g.n[0] * jy], qy * wt[0][a]);
+                atomicAdd(&rho[jx + g.n[0] * jy], (double)(qy * wt[0][a]));
             }
         }
     } else {
@@ -46,45 +47,61 @@ __global__ void __launch_bounds__(256) k_deposit_particles(PartP<T> p, GridP<T> 
 #pragma unroll
                 for (int a = 0; a <= P; ++a) {
                     const int jx = fold(first[0] + a, g.n[0]);
-                    atomicAdd(&rho[row + jx], qy * wt[0][a]);
+                    atomicAdd(&rho[row + jx], (double)(qy * wt[0][a]));
                 }
             }
         }
     }
 }
 
+// rho is accumulated in double (racc): directly in rho for fp64 grids, in the workspace grid for
+// fp32 grids, which is then rounded once -- so the fp32 result does not depend on how many
+// addends a node receives (clustered config 4) or on the order of the atomics.
 template <typename T, int D, int P>
-static int deposit_impl(const pic_grid_t& g, const pic_particles_t& p, void* rho, cudaStream_t st)
+static int deposit_impl(const pic_grid_t& g, const pic_particles_t& p, int order_state, const int32_t* cell_offsets,
+                        void* rho, double* racc_ws, cudaStream_t st)
 {
     int64_t C = 1;
     for (int c = 0; c < g.dim; ++c) C *= g.n[c];
-    PIC_CUDA_OK(cudaMemsetAsync(rho, 0, sizeof(T) * (size_t)C, st));
+    double* racc = sizeof(T) == 8 ? (double*)rho : racc_ws;
+    if (!racc) return PIC_ERR_WORKSPACE;
+    PIC_CUDA_OK(cudaMemsetAsync(racc, 0, sizeof(double) * (size_t)C, st));
     if (p.n > 0) {
-        k_deposit_particles<T, D, P><<<(unsigned)((p.n + 255) / 256), 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g),
-                                                                                   p.n, (T*)rho);
+        if (order_state == PIC_ORDER_SORTED) {
+            int rc = launch_cells<T, D, P, kModeDeposit, 8, (sizeof(T) == 4 ? 2 : 1), false>(g, p, p, nullptr, cell_offsets, nullptr, racc, 0.0, 0.0, st);
+            if (rc != PIC_OK) return rc;
+        } else {
+            k_deposit_particles<T, D, P><<<(unsigned)((p.n + 255) / 256), 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g),
+                                                                                       p.n, racc);
+            count_launch();
+        }
+    }
+    if (sizeof(T) == 4) {
+        k_round_rho<T><<<(unsigned)((C + 255) / 256), 256, 0, st>>>(racc, (T*)rho, C);
         count_launch();
     }
     return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
 
 template <typename T, int D>
-static int deposit_order(const pic_grid_t& g, const pic_particles_t& p, void* rho, cudaStream_t st)
+static int deposit_order(const pic_grid_t& g, const pic_particles_t& p, int order_state, const int32_t* cell_offsets,
+                         void* rho, double* racc, cudaStream_t st)
 {
     switch (g.order) {
-    case 1: return deposit_impl<T, D, 1>(g, p, rho, st);
-    case 2: return deposit_impl<T, D, 2>(g, p, rho, st);
-    default: return deposit_impl<T, D, 3>(g, p, rho, st);
+    case 1: return deposit_impl<T, D, 1>(g, p, order_state, cell_offsets, rho, racc, st);
+    case 2: return deposit_impl<T, D, 2>(g, p, order_state, cell_offsets, rho, racc, st);
+    default: return deposit_impl<T, D, 3>(g, p, order_state, cell_offsets, rho, racc, st);
     }
 }
 
 int launch_deposit(const pic_grid_t& g, const pic_particles_t& p, int order_state, const int32_t* cell_offsets,
-                   void* rho, cudaStream_t st)
+                   void* rho, double* racc, cudaStream_t st)
 {
-    (void)order_state;
-    (void)cell_offsets;
     if (g.dtype == PIC_F32)
-        return g.dim == 2 ? deposit_order<float, 2>(g, p, rho, st) : deposit_order<float, 3>(g, p, rho, st);
-    return g.dim == 2 ? deposit_order<double, 2>(g, p, rho, st) : deposit_order<double, 3>(g, p, rho, st);
+        return g.dim == 2 ? deposit_order<float, 2>(g, p, order_state, cell_offsets, rho, racc, st)
+                          : deposit_order<float, 3>(g, p, order_state, cell_offsets, rho, racc, st);
+    return g.dim == 2 ? deposit_order<double, 2>(g, p, order_state, cell_offsets, rho, racc, st)
+                      : deposit_order<double, 3>(g, p, order_state, cell_offsets, rho, racc, st);
 }
 
 }  // namespace pic

@@ -8,14 +8,9 @@
 // and counts 6 loads + 3 stores for each; fused they are
 // 2d loads + 2d stores per particle.  k_push_particles reads E through the read-only path
 // ("scattered reads through read-only data cache") and is correct for any order.
-#include "pic_common.cuh"
+#include "pic_cells.cuh"
 
 namespace pic {
-
-template <typename T>
-struct FieldP {
-    const T* E[3];
-};
 
 template <typename T, int D, int P>
 __global__ void __launch_bounds__(256) k_push_particles(PartP<T> p, GridP<T> g, FieldP<T> f, int64_t n, T dt, T qmdt)
@@ -64,10 +59,12 @@ __global__ void __launch_bounds__(256) k_push_particles(PartP<T> p, GridP<T> g, 
 }
 
 template <typename T, int D, int P>
-static int push_impl(const pic_grid_t& g, pic_particles_t& p, const void* const E[3], double dt, double qm,
-                     cudaStream_t st)
+static int push_impl(const pic_grid_t& g, pic_particles_t& p, int order_state, const int32_t* cell_offsets,
+                     const void* const E[3], double dt, double qm, cudaStream_t st)
 {
     if (p.n > 0) {
+        if (order_state == PIC_ORDER_SORTED)
+            return launch_cells<T, D, P, kModePush, 8, (sizeof(T) == 4 ? 2 : 1), false>(g, p, p, nullptr, cell_offsets, E, nullptr, dt, qm, st);
         FieldP<T> f;
         for (int c = 0; c < 3; ++c) f.E[c] = c < D ? (const T*)E[c] : nullptr;
         k_push_particles<T, D, P><<<(unsigned)((p.n + 255) / 256), 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), f, p.n,
@@ -78,24 +75,24 @@ static int push_impl(const pic_grid_t& g, pic_particles_t& p, const void* const 
 }
 
 template <typename T, int D>
-static int push_order(const pic_grid_t& g, pic_particles_t& p, const void* const E[3], double dt, double qm,
-                      cudaStream_t st)
+static int push_order(const pic_grid_t& g, pic_particles_t& p, int order_state, const int32_t* cell_offsets,
+                      const void* const E[3], double dt, double qm, cudaStream_t st)
 {
     switch (g.order) {
-    case 1: return push_impl<T, D, 1>(g, p, E, dt, qm, st);
-    case 2: return push_impl<T, D, 2>(g, p, E, dt, qm, st);
-    default: return push_impl<T, D, 3>(g, p, E, dt, qm, st);
+    case 1: return push_impl<T, D, 1>(g, p, order_state, cell_offsets, E, dt, qm, st);
+    case 2: return push_impl<T, D, 2>(g, p, order_state, cell_offsets, E, dt, qm, st);
+    default: return push_impl<T, D, 3>(g, p, order_state, cell_offsets, E, dt, qm, st);
     }
 }
 
 int launch_push(const pic_grid_t& g, pic_particles_t& p, int order_state, const int32_t* cell_offsets,
                 const void* const E[3], double dt, double qm, cudaStream_t st)
 {
-    (void)order_state;
-    (void)cell_offsets;
     if (g.dtype == PIC_F32)
-        return g.dim == 2 ? push_order<float, 2>(g, p, E, dt, qm, st) : push_order<float, 3>(g, p, E, dt, qm, st);
-    return g.dim == 2 ? push_order<double, 2>(g, p, E, dt, qm, st) : push_order<double, 3>(g, p, E, dt, qm, st);
+        return g.dim == 2 ? push_order<float, 2>(g, p, order_state, cell_offsets, E, dt, qm, st)
+                          : push_order<float, 3>(g, p, order_state, cell_offsets, E, dt, qm, st);
+    return g.dim == 2 ? push_order<double, 2>(g, p, order_state, cell_offsets, E, dt, qm, st)
+                      : push_order<double, 3>(g, p, order_state, cell_offsets, E, dt, qm, st);
 }
 
 }  // namespace pic

@@ -340,7 +340,7 @@ static int64_t cells_of(const pic_grid_t& g)
 }
 
 struct SortLayout {
-    size_t keys0, keys1, idx0, idx1, zero_begin, cell_count, digit_hist, scan_status, counters, lookback, total;
+    size_t keys0, keys1, idx0, idx1, zero_begin, cell_count, digit_hist, scan_status, counters, lookback, zero_end, racc, total;
     int passes, bits, key_bits;
     int64_t radix_tiles, scan_tiles;
 };
@@ -366,6 +366,8 @@ static SortLayout sort_layout(const pic_grid_t& g, int64_t n)
     L.scan_status = off; off += align256(sizeof(uint32_t) * (size_t)L.scan_tiles);
     L.counters = off; off += 256;
     L.lookback = off; off += align256(sizeof(uint32_t) * (size_t)L.passes * (size_t)(L.radix_tiles > 0 ? L.radix_tiles : 1) * kRadix);
+    L.zero_end = off;
+    L.racc = off; off += align256(sizeof(double) * (size_t)C);
     L.total = off;
     return L;
 }
@@ -387,7 +389,8 @@ int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, Sor
     o.counters = (uint32_t*)(b + L.counters);
     o.lookback = (uint32_t*)(b + L.lookback);
     o.zero_begin = b + L.zero_begin;
-    o.zero_bytes = L.total - L.zero_begin;
+    o.zero_bytes = L.zero_end - L.zero_begin;
+    o.racc = (double*)(b + L.racc);
     o.passes = L.passes;
     o.bits_per_pass = L.bits;
     o.key_bits = L.key_bits;
@@ -438,12 +441,12 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
 
 template <typename T, int D>
 static int sort_impl(const pic_grid_t& g, const pic_particles_t& in, pic_particles_t& out, int32_t* perm,
-                     int32_t* cell_offsets, const SortWs& ws, cudaStream_t st)
+                     int32_t* cell_offsets, const SortWs& ws, bool reorder, cudaStream_t st)
 {
     int rc = sort_keys_perm<T, D>(g, in, perm, cell_offsets, ws, st);
     if (rc != PIC_OK) return rc;
     const int64_t n = in.n;
-    if (n > 0) {
+    if (n > 0 && reorder) {
         k_reorder<T, D><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(make_partp<T>(in), make_partp<T>(out), perm, n);
         count_launch();
     }
@@ -452,14 +455,14 @@ static int sort_impl(const pic_grid_t& g, const pic_particles_t& in, pic_particl
 }
 
 int launch_sort(const pic_grid_t& g, const pic_particles_t& in, pic_particles_t& out, int32_t* perm,
-                int32_t* cell_offsets, const SortWs& ws, cudaStream_t st)
+                int32_t* cell_offsets, const SortWs& ws, bool reorder, cudaStream_t st)
 {
     if (g.dtype == PIC_F32) {
-        return g.dim == 2 ? sort_impl<float, 2>(g, in, out, perm, cell_offsets, ws, st)
-                          : sort_impl<float, 3>(g, in, out, perm, cell_offsets, ws, st);
+        return g.dim == 2 ? sort_impl<float, 2>(g, in, out, perm, cell_offsets, ws, reorder, st)
+                          : sort_impl<float, 3>(g, in, out, perm, cell_offsets, ws, reorder, st);
     }
-    return g.dim == 2 ? sort_impl<double, 2>(g, in, out, perm, cell_offsets, ws, st)
-                      : sort_impl<double, 3>(g, in, out, perm, cell_offsets, ws, st);
+    return g.dim == 2 ? sort_impl<double, 2>(g, in, out, perm, cell_offsets, ws, reorder, st)
+                      : sort_impl<double, 3>(g, in, out, perm, cell_offsets, ws, reorder, st);
 }
 
 }  // namespace pic

@@ -122,14 +122,14 @@ def test_deposit_parity(name, kw, order):
     rho_ref = O.deposit(go, wl.x, wl.w)
     x, w = to_dev(wl.x), to_dev([wl.w])[0]
     rho = torch.full((gb.cells,), 123.0, dtype=gb.torch_dtype, device="cuda")      # must be overwritten
-    B.pic_deposit(gb, x, w, rho, B.PIC_ORDER_UNSORTED)
+    ws = torch.empty(B.pic_workspace_bytes(gb, cfg.N), dtype=torch.uint8, device="cuda")
+    B.pic_deposit(gb, x, w, rho, B.PIC_ORDER_UNSORTED, None, ws)
     assert err_rho(rho.cpu().numpy(), rho_ref) <= TOL_RHO[cfg.dtype]
     # sorted path
     xs, vs, wsrt, perm, off = O.sort(go, wl.x, wl.v, wl.w)
     rho_ref_s = O.deposit(go, xs, wsrt)
     xd, wd = to_dev(xs), to_dev([wsrt])[0]
     offd = torch.from_numpy(np.concatenate([off, np.zeros(3, np.int32)])).cuda()
-    ws = torch.empty(B.pic_workspace_bytes(gb, cfg.N), dtype=torch.uint8, device="cuda")
     rho.fill_(-7.0)
     B.pic_deposit(gb, xd, wd, rho, B.PIC_ORDER_SORTED, offd, ws)
     r = rho.cpu().numpy()
