@@ -79,12 +79,13 @@ __device__ __forceinline__ T grid_coord(T x, T h, T inv_h, int hmul)
 }
 
 // Clamped cell index: "if (ix<0) ix=0; if (ix>nx-1) ix=nx-1".
+// floor() by a saturating round-down conversion (NaN -> 0), then an integer clamp: no branches.
+__device__ __forceinline__ int floor_to_int(float t) { return __float2int_rd(t); }
+__device__ __forceinline__ int floor_to_int(double t) { return __double2int_rd(t); }
 template <typename T>
 __device__ __forceinline__ int cell_index(T t, int n)
 {
-    T f = floor(t);
-    int i = (f < (T)0) ? 0 : ((f > (T)(n - 1)) ? n - 1 : (int)f);
-    return i;
+    return max(0, min(floor_to_int(t), n - 1));
 }
 
 // One-dimensional stencil of degree P: first (unfolded) node and the P+1 weights.
@@ -148,18 +149,29 @@ void mark_phase(int phase, cudaStream_t st);
 
 // ---- launchers implemented in the .cu files (all enqueue on `st`) ------------------------
 struct SortWs {
-    uint32_t* keys[2];
-    uint32_t* idx[2];
-    int32_t* cell_count;     // [C]
+    uint32_t* keys[2];       // [N] movers' keys, ping-pong
+    uint32_t* idx[2];        // [N] movers' positions, ping-pong
+    uint32_t* mask;          // [N/32 + 2] mover bit of every position
+    uint32_t* mprefix;       // [N/32 + 2] movers before each 32-position word
+    int32_t* old_off;        // [C+1] the hint: cell_offsets as found on entry
+    int32_t* mover_off;      // [C+1] exclusive scan of mover_count
+    int32_t* cell_base;      // [C]   where the stayers of a cell start in perm (see k_cell_base)
+    int32_t* tile_first;     // [classify tiles] first cell of every classify tile
+    int32_t* tile_count;     // [classify tiles] movers per tile
+    int32_t* tile_base;      // [classify tiles + 1] exclusive scan of tile_count
+    uint32_t* lookback;      // [passes][radix tiles][kRadix]
+    int32_t* cell_count;     // [C+1] histogram of the keys              (zero region from here ...)
+    int32_t* mover_count;    // [C+1] histogram of the movers' keys
+    int32_t* mover_lo;       // [C+1] movers into a cell from below its hint interval
     uint32_t* digit_hist;    // [kMaxPasses][kRadix]
-    uint32_t* scan_status;   // [scan tiles]
-    uint32_t* counters;      // [16]
-    uint32_t* lookback;      // [passes][tiles][kRadix]
+    uint32_t* scan_status;   // [2][scan tiles]
+    uint32_t* cls_status;    // [scan tiles of the classify tiles]
+    uint32_t* counters;      // [64] tile tickets, number of movers, hint flag  (... to here)
     double* racc;            // [C] double accumulation grid of the deposit (not in the zero region)
     void* zero_begin;        // region that must be zero before a sort
     size_t zero_bytes;
     int passes, bits_per_pass, key_bits;
-    int64_t radix_tiles, scan_tiles;
+    int64_t radix_tiles, scan_tiles, cls_tiles;
 };
 
 size_t sort_ws_bytes(const pic_grid_t& g, int64_t n);

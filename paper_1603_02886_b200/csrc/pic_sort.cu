@@ -1,18 +1,35 @@
 // pic_sort.cu -- stable counting sort of the particles by cell key (rows a1-a4 of the hot path).
 //
 // The paper sorts with histogram -> prefix sum -> atomic-counter scatter (section 3.2,
-// Alg. 2 lines 1-5 PAPER.md:207-212) and notes that hand-written CUDA histogram and prefix-sum
-// kernels were worth a factor 2.  The atomic scatter is not stable; this
-// build needs the unique stable permutation (R7), so the scatter is an LSD radix sort of
-// (key, source index) pairs, each pass a one-sweep partition: warp-aggregated ranking, per-tile
-// digit counts chained by decoupled look-back, coalesced scatter from a shared-memory staging
-// tile.  The full-key histogram and its exclusive scan give cell_offsets.
+// Alg. 2 lines 1-5 PAPER.md:207-212), notes that hand-written CUDA histogram and prefix-sum
+// kernels were worth a factor 2, and prefers, "for the rest of this paper", a
+// sort for PRE-ORDERED particles that only moves the particles whose bucket changed (Alg. 2,
+// PAPER.md:124, 190-196, 207-258; 23 % of the particles per step).  The atomic scatter
+// is not stable; this build needs the unique stable permutation (R7).  It gets it from the same
+// two ideas:
 //
-// Kernels:  k_keys_hist      x[d] -> key, full-key histogram (run-aggregated atomics), digit histograms
-//           k_scan_cells     count[C] -> cell_offsets[C+1]   (single pass, decoupled look-back)
+//   * cell_offsets as found ON ENTRY is read as a hint: intervals I_k = [hint[k], hint[k+1]) that
+//     described the order of `in` at some earlier time (the previous step's output).  A particle
+//     at position i is a STAYER if i lies in the interval of its NEW key, else a MOVER.  For any
+//     non-decreasing hint the stable order of cell k is: movers into k from positions below I_k
+//     (ascending position), the stayers of k (ascending position), movers from above I_k.  So only
+//     the movers are sorted: they are compacted in position order (decoupled look-back) and go
+//     through an LSD radix sort of (key, position) pairs, each pass a one-sweep stable partition
+//     (warp-aggregated ranking, per-tile digit counts chained by decoupled look-back).  A hint that
+//     is not non-decreasing within [0, N] (first call, garbage) makes every particle a mover: the
+//     result is the same permutation, only slower.
+//   * the full-key histogram and its exclusive scan give cell_offsets; the movers' histogram and
+//     its scan place each mover inside its cell.
+//
+// Kernels:  k_hint_check     hint -> private copy, validity flag
+//           k_hint_tiles     first cell of every 4096-position tile (for k_perm_stayers)
+//           k_classify       x[d] -> key, histograms, stayer/mover split, movers compacted in order
+//           k_scan_cells     count[C] -> exclusive offsets [C+1] (single pass, decoupled look-back)
 //           k_scan_digits    digit histograms -> exclusive global digit offsets
-//           k_radix_pass     one stable partition by an 8-bit digit
-//           k_reorder        out_a[j] = in_a[perm[j]] for every attribute
+//           k_radix_pass     one stable partition of the movers by an (at most) 8-bit digit
+//           k_cell_base      per cell: where its stayers start in perm
+//           k_perm_movers / k_perm_stayers   perm
+//           k_reorder        out_a[j] = in_a[perm[j]] for every attribute (pic_sort only)
 #include <cmath>
 
 #include "pic_common.cuh"
@@ -31,7 +48,15 @@ constexpr int kScanThreads = 256;
 constexpr int kScanIPT = 8;
 constexpr int kScanTile = kScanThreads * kScanIPT;         // 2048 counts per tile
 
+constexpr int kClsThreads = 256;
+constexpr int kClsIPT = 16;
+constexpr int kClsTile = kClsThreads * kClsIPT;            // 4096 positions per tile
+constexpr int kClsWarps = kClsThreads / 32;
+
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagPrefix = 2u << 30, kValMask = (1u << 30) - 1;
+
+// slots of SortWs::counters
+enum { kCtrScanA = 0, kCtrScanB = 1, kCtrCls = 2, kCtrRadix = 3 /* .. +kMaxPasses */, kCtrMovers = 8, kCtrHintBad = 9 };
 
 __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p)
 {
@@ -42,48 +67,208 @@ __device__ __forceinline__ void st_volatile(uint32_t* p, uint32_t v)
     *reinterpret_cast<volatile uint32_t*>(p) = v;
 }
 
-// ----------------------------------------------------------------------------- keys + histograms
+// look-back of a single-value chain by one warp: returns the exclusive prefix of `tile`
+__device__ __forceinline__ uint32_t warp_lookback(uint32_t* status, int tile, uint32_t total, unsigned lane)
+{
+    if (lane == 0) st_volatile(&status[tile], (tile == 0 ? kFlagPrefix : kFlagAgg) | total);
+    uint32_t excl = 0;
+    int look = tile - 1;
+    while (look >= 0) {
+        int t = look - (int)lane;
+        uint32_t s;
+        do {
+            s = (t >= 0) ? ld_volatile(&status[t]) : kFlagPrefix;
+        } while (__any_sync(0xFFFFFFFFu, (s >> 30) == 0));
+        unsigned pref = __ballot_sync(0xFFFFFFFFu, (s >> 30) == 2);
+        int stop = pref ? __ffs(pref) - 1 : 31;            // nearest predecessor with an inclusive prefix
+        uint32_t contrib = ((int)lane <= stop) ? (s & kValMask) : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xFFFFFFFFu, contrib, o);
+        excl += contrib;
+        if (pref) break;
+        look -= 32;
+    }
+    if (lane == 0 && tile != 0) st_volatile(&status[tile], kFlagPrefix | (excl + total));
+    return excl;
+}
+
+// ----------------------------------------------------------------------------- the hint
+// private copy of cell_offsets as found on entry; bad = 1 unless 0 <= h[0] <= h[1] <= ... <= h[C] <= N
+__global__ void __launch_bounds__(256) k_hint_check(const int32_t* __restrict__ hint, int32_t* __restrict__ old_off, int C,
+                                                    int64_t n, uint32_t* counters)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k > C) return;
+    const int32_t a = hint[k];
+    old_off[k] = a;
+    bool bad = a < 0 || (int64_t)a > n;
+    if (k < C) bad = bad || hint[k + 1] < a;
+    if (bad) counters[kCtrHintBad] = 1u;
+}
+
+// tile_first[t] = smallest k with old_off[k+1] > t*kClsTile (C if none): the first cell whose
+// interval can hold a position of tile t.  One thread per cell; the loop lengths add up to
+// (#tiles + C) because the hint is non-decreasing (the kernel does nothing for a bad hint).
+__global__ void __launch_bounds__(256) k_hint_tiles(const int32_t* __restrict__ old_off, int C, int ntiles,
+                                                    int32_t* __restrict__ tile_first, const uint32_t* __restrict__ counters)
+{
+    if (counters[kCtrHintBad]) return;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k > C) return;
+    // tiles t with b_{k-1} <= t*kClsTile < b_k, where b_k = old_off[k+1], b_{-1} = 0, b_C = +inf
+    const int64_t lo = k == 0 ? 0 : old_off[k];
+    const int64_t hi = k == C ? (int64_t)ntiles * kClsTile : old_off[k + 1];
+    for (int64_t t = (lo + kClsTile - 1) / kClsTile; t * kClsTile < hi && t < ntiles; ++t) tile_first[t] = k;
+}
+
+// ----------------------------------------------------------------------------- keys, histograms, stayer/mover split
 // a1: key = c_x + n_x*(c_y + n_y*c_z) (x fastest), clamped cell index
 // (PAPER.md:493-497).  a2: count[key]++ -- consecutive lanes holding the same key (the common
 // case once the particles are pre-ordered) are merged into one atomic per run.
+// Movers (see the header) are appended to (mkey, midx) in position order; mask / mprefix hold,
+// per 32 positions, the movers' bits and the number of movers before the word.
 template <typename T, int D>
-__global__ void __launch_bounds__(256) k_keys_hist(PartP<T> p, GridP<T> g, int64_t n, uint32_t* __restrict__ key_out,
-                                                   int32_t* __restrict__ cell_count)
+__global__ void __launch_bounds__(kClsThreads)
+k_classify(PartP<T> p, GridP<T> g, int64_t n, const int32_t* __restrict__ old_off, int32_t* __restrict__ cell_count,
+           int32_t* __restrict__ mover_count, int32_t* __restrict__ mover_lo, uint32_t* __restrict__ mkey,
+           uint32_t* __restrict__ midx, uint32_t* __restrict__ mask, uint32_t* __restrict__ mprefix,
+           int32_t* __restrict__ tile_count, const uint32_t* __restrict__ counters)
 {
-    const unsigned lane = threadIdx.x & 31;
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    const int64_t n_round = (n + 31) & ~(int64_t)31;          // keep warps converged for the shuffles
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
-        const bool valid = i < n;
-        uint32_t key = 0xFFFFFFFFu;
-        if (valid) {
+    __shared__ uint32_t s_wsum[kClsWarps];
+    const unsigned tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tile = (int)blockIdx.x;
+    const bool hint_ok = counters[kCtrHintBad] == 0u;
+    const int64_t wbase = (int64_t)tile * kClsTile + warp * (32 * kClsIPT);
+
+    // all positions of this thread first: independent loads
+    T xs[D][kClsIPT];
+#pragma unroll
+    for (int r = 0; r < kClsIPT; ++r) {
+        const int64_t i = wbase + r * 32 + lane;
+#pragma unroll
+        for (int c = 0; c < D; ++c) xs[c][r] = i < n ? p.x[c][i] : (T)0;
+    }
+    uint32_t key[kClsIPT], bal[kClsIPT];
+    uint32_t mover_bits = 0, lo_bits = 0;
+#pragma unroll
+    for (int r = 0; r < kClsIPT; ++r) {
+        const int64_t i = wbase + r * 32 + lane;
+        key[r] = 0xFFFFFFFFu;
+        if (i < n) {
             int k = 0, mul = 1;
 #pragma unroll
             for (int c = 0; c < D; ++c) {
-                T t = grid_coord(p.x[c][i], g.h[c], g.inv_h[c], g.hmul);
+                T t = grid_coord(xs[c][r], g.h[c], g.inv_h[c], g.hmul);
                 k += mul * cell_index(t, g.n[c]);
                 mul *= g.n[c];
             }
-            key = (uint32_t)k;
-            key_out[i] = key;
+            key[r] = (uint32_t)k;
         }
-        // run-length aggregation inside the warp
-        uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, key, 1);
-        bool head = (lane == 0) || (prev != key);
-        unsigned heads = __ballot_sync(0xFFFFFFFFu, head);
+    }
+    // the hint intervals of the new keys: independent loads again
+    if (hint_ok) {
+        int32_t ha[kClsIPT], hb[kClsIPT];
+#pragma unroll
+        for (int r = 0; r < kClsIPT; ++r) {
+            const bool valid = key[r] != 0xFFFFFFFFu;
+            ha[r] = valid ? old_off[key[r]] : 0;
+            hb[r] = valid ? old_off[key[r] + 1] : 0;
+        }
+#pragma unroll
+        for (int r = 0; r < kClsIPT; ++r) {
+            const int64_t i = wbase + r * 32 + lane;
+            if (key[r] != 0xFFFFFFFFu) {
+                if (!((int64_t)ha[r] <= i && i < (int64_t)hb[r])) mover_bits |= 1u << r;
+                if (i < (int64_t)ha[r]) lo_bits |= 1u << r;
+            }
+        }
+    } else {
+#pragma unroll
+        for (int r = 0; r < kClsIPT; ++r)
+            if (key[r] != 0xFFFFFFFFu) mover_bits |= 1u << r;
+    }
+#pragma unroll
+    for (int r = 0; r < kClsIPT; ++r) {
+        // run-length aggregation of the histogram inside the warp
+        const bool valid = key[r] != 0xFFFFFFFFu;
+        const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, key[r], 1);
+        const bool head = (lane == 0) || (prev != key[r]);
+        const unsigned heads = __ballot_sync(0xFFFFFFFFu, head);
         if (head && valid) {
-            unsigned above = heads & ~((2u << lane) - 1);      // heads strictly above this lane
-            int next = above ? __ffs(above) - 1 : 32;
-            atomicAdd(&cell_count[key], next - (int)lane);
+            const unsigned above = heads & ~((2u << lane) - 1);      // heads strictly above this lane
+            const int next = above ? __ffs(above) - 1 : 32;
+            // a run never extends over the invalid lanes of a ragged last word: those carry key
+            // 0xFFFFFFFF, so the first of them is a head
+            atomicAdd(&cell_count[key[r]], next - (int)lane);
+        }
+        bal[r] = __ballot_sync(0xFFFFFFFFu, (mover_bits >> r) & 1u);
+    }
+    // movers before each word of this warp, warp total
+    uint32_t wpre[kClsIPT], wtotal = 0;
+#pragma unroll
+    for (int r = 0; r < kClsIPT; ++r) { wpre[r] = wtotal; wtotal += __popc(bal[r]); }
+    if (lane == 0) s_wsum[warp] = wtotal;
+    __syncthreads();
+    uint32_t warp_off = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < kClsWarps; ++w) {
+        const uint32_t t = s_wsum[w];
+        if (w < (int)warp) warp_off += t;
+        total += t;
+    }
+    if (tid == 0) tile_count[tile] = (int32_t)total;
+    // tile-relative for now: k_movers_place adds the movers of the tiles before this one
+    const uint32_t base = warp_off;
+    const int64_t stage = (int64_t)tile * kClsTile;
+    const unsigned lt = (1u << lane) - 1;
+#pragma unroll
+    for (int r = 0; r < kClsIPT; ++r) {
+        const int64_t i0 = wbase + r * 32;
+        if (i0 < n && lane == 0) {
+            mask[i0 >> 5] = bal[r];
+            mprefix[i0 >> 5] = base + wpre[r];
+        }
+        if ((mover_bits >> r) & 1u) {
+            const int64_t dst = stage + base + wpre[r] + __popc(bal[r] & lt);
+            mkey[dst] = key[r];
+            midx[dst] = (uint32_t)(i0 + lane);
+            atomicAdd(&mover_count[key[r]], 1);
+            if ((lo_bits >> r) & 1u) atomicAdd(&mover_lo[key[r]], 1);
         }
     }
 }
 
-// ----------------------------------------------------------------------------- exclusive scan of the cell counts
-// a3: cell_offsets[k] = sum_{k'<k} count[k'], cell_offsets[C] = N ("prefix sum").
+// The movers of tile t, staged by k_classify at [t*kClsTile, ...), move to their place in the global
+// list: tile_base[t] = number of movers in the tiles before t (exclusive scan of tile_count).  The
+// per-word mover prefixes become global too.
+__global__ void __launch_bounds__(kClsThreads)
+k_movers_place(const uint32_t* __restrict__ stage_key, const uint32_t* __restrict__ stage_idx, uint32_t* __restrict__ mkey,
+               uint32_t* __restrict__ midx, uint32_t* __restrict__ mask, uint32_t* __restrict__ mprefix,
+               const int32_t* __restrict__ tile_base, int ntiles, int64_t n, uint32_t* counters)
+{
+    const int tile = (int)blockIdx.x, tid = threadIdx.x;
+    const uint32_t base = (uint32_t)tile_base[tile];
+    const int cnt = tile_base[tile + 1] - tile_base[tile];
+    const int64_t stage = (int64_t)tile * kClsTile;
+    for (int r = tid; r < cnt; r += kClsThreads) {
+        mkey[base + r] = stage_key[stage + r];
+        midx[base + r] = stage_idx[stage + r];
+    }
+    const int64_t w0 = stage >> 5, nwords = (n + 31) / 32;
+    for (int w = tid; w < kClsTile / 32 && w0 + w < nwords; w += kClsThreads) mprefix[w0 + w] += base;
+    if (tile == ntiles - 1 && tid == 0) {                // total number of movers, sentinel word
+        const uint32_t total = (uint32_t)tile_base[ntiles];
+        counters[kCtrMovers] = total;
+        mask[nwords] = 0u;
+        mprefix[nwords] = total;
+    }
+}
+
+// ----------------------------------------------------------------------------- exclusive scan of per-cell counts
+// a3: offsets[k] = sum_{k'<k} count[k'], offsets[C] = total ("prefix sum").
 // Single pass: each tile publishes its aggregate, then looks back over its predecessors.
-// The per-pass digit histograms of the radix sort are summed here from the cell counts
-// (C cells instead of N particles).
+// With digit_hist != NULL the per-pass digit histograms of the radix sort are summed here from
+// the counts (C cells instead of one pass over the keys).
 __global__ void __launch_bounds__(kScanThreads) k_scan_cells(const int32_t* __restrict__ count, int32_t* __restrict__ offsets,
                                                               int C, uint32_t* status, uint32_t* tile_counter,
                                                               uint32_t* __restrict__ digit_hist, int passes, int bits)
@@ -92,7 +277,8 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_cells(const int32_t* __re
     __shared__ uint32_t s_tile, s_excl;
     __shared__ uint32_t s_hist[kMaxPasses][kRadix];
     if (threadIdx.x == 0) s_tile = atomicAdd(tile_counter, 1u);
-    for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += kScanThreads) (&s_hist[0][0])[i] = 0;
+    if (digit_hist)
+        for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += kScanThreads) (&s_hist[0][0])[i] = 0;
     __syncthreads();
     const int tile = (int)s_tile;
     const int base = tile * kScanTile + threadIdx.x * kScanIPT;
@@ -105,7 +291,7 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_cells(const int32_t* __re
         v[k] = (base + k < C) ? (uint32_t)count[base + k] : 0u;
         sum += v[k];
     }
-    {
+    if (digit_hist) {
         const uint32_t mask = (1u << bits) - 1;
         for (int q = 0; q < passes; ++q) {
 #pragma unroll
@@ -131,30 +317,9 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_cells(const int32_t* __re
     }
     uint32_t excl_thread = warp_off + inc - sum;
 
-    // decoupled look-back, done by warp 0
     if (warp == 0) {
-        if (lane == 0) st_volatile(&status[tile], (tile == 0 ? kFlagPrefix : kFlagAgg) | total);
-        uint32_t excl = 0;
-        int look = tile - 1;
-        while (look >= 0) {
-            int t = look - (int)lane;
-            uint32_t s;
-            do {
-                s = (t >= 0) ? ld_volatile(&status[t]) : kFlagPrefix;
-            } while (__any_sync(0xFFFFFFFFu, (s >> 30) == 0));
-            unsigned pref = __ballot_sync(0xFFFFFFFFu, (s >> 30) == 2);
-            int stop = pref ? __ffs(pref) - 1 : 31;            // nearest predecessor with an inclusive prefix
-            uint32_t contrib = ((int)lane <= stop) ? (s & kValMask) : 0u;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xFFFFFFFFu, contrib, o);
-            excl += contrib;
-            if (pref) break;
-            look -= 32;
-        }
-        if (lane == 0) {
-            if (tile != 0) st_volatile(&status[tile], kFlagPrefix | (excl + total));
-            s_excl = excl;
-        }
+        const uint32_t excl = warp_lookback(status, tile, total, lane);
+        if (lane == 0) s_excl = excl;
     }
     __syncthreads();
     uint32_t run = s_excl + excl_thread;
@@ -164,9 +329,11 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_cells(const int32_t* __re
         run += v[k];
         if (base + k == C - 1) offsets[C] = (int32_t)run;
     }
-    for (int i = threadIdx.x; i < passes * kRadix; i += kScanThreads) {
-        uint32_t c = (&s_hist[0][0])[i];
-        if (c) atomicAdd(&digit_hist[i], c);
+    if (digit_hist) {
+        for (int i = threadIdx.x; i < passes * kRadix; i += kScanThreads) {
+            uint32_t c = (&s_hist[0][0])[i];
+            if (c) atomicAdd(&digit_hist[i], c);
+        }
     }
 }
 
@@ -189,15 +356,27 @@ __global__ void __launch_bounds__(kRadix) k_scan_digits(uint32_t* digit_hist)
     h[threadIdx.x] = off + inc - c;
 }
 
-// ----------------------------------------------------------------------------- one radix pass
+// zero the look-back words the radix passes will use: passes x tiles(number of movers) x kRadix
+__global__ void __launch_bounds__(256) k_zero_lookback(uint32_t* lookback, const uint32_t* __restrict__ counters, int passes,
+                                                       int64_t pass_stride)
+{
+    const int64_t tiles = ((int64_t)counters[kCtrMovers] + kRadixTile - 1) / kRadixTile;
+    const int64_t words = tiles * kRadix;
+    for (int q = 0; q < passes; ++q)
+        for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < words; i += (int64_t)gridDim.x * blockDim.x)
+            lookback[q * pass_stride + i] = 0u;
+}
+
+// ----------------------------------------------------------------------------- one radix pass over the movers
 // Stable partition of (key, idx) pairs by digit (key >> shift) & mask (at most 8 bits).  Tile-local order is
 // (warp, round, lane) = ascending input position, so equal digits keep their input order.
-// idx_in == nullptr: idx is the input position (first pass).  keys_out == nullptr: keys are
-// not needed any more (last pass).
+// keys_out == nullptr: keys are not needed any more (last pass).  The number of pairs is read
+// from the device (counters[kCtrMovers]); blocks beyond the last tile exit at once.
 __global__ void __launch_bounds__(kRadixThreads)
 k_radix_pass(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ idx_in,
-             uint32_t* __restrict__ keys_out, uint32_t* __restrict__ idx_out, int64_t n, int shift, uint32_t mask,
-             const uint32_t* __restrict__ digit_offsets, uint32_t* tile_counter, uint32_t* lookback)
+             uint32_t* __restrict__ keys_out, uint32_t* __restrict__ idx_out, const uint32_t* __restrict__ counters,
+             int shift, uint32_t mask, const uint32_t* __restrict__ digit_offsets, uint32_t* tile_counter,
+             uint32_t* lookback)
 {
     __shared__ uint32_t s_cnt[kRadixWarps][kRadix];   // per-warp digit counters -> per-warp bases
     __shared__ uint32_t s_start[kRadix];              // tile-local start of each digit
@@ -207,6 +386,8 @@ k_radix_pass(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ 
     __shared__ uint32_t s_wsum[kRadixWarps];
     __shared__ uint32_t s_tile;
 
+    const int64_t n = counters[kCtrMovers];
+    if ((int64_t)blockIdx.x * kRadixTile >= n) return;   // as many blocks run as there are tiles
     const unsigned tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_tile = atomicAdd(tile_counter, 1u);
     for (int i = tid; i < kRadixWarps * kRadix; i += kRadixThreads) (&s_cnt[0][0])[i] = 0;
@@ -224,7 +405,7 @@ k_radix_pass(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ 
         int loc = wbase + r * 32;
         bool ok = loc < tile_valid;
         key[r] = ok ? keys_in[tile_base + loc] : 0xFFFFFFFFu;
-        val[r] = ok ? (idx_in ? idx_in[tile_base + loc] : (uint32_t)(tile_base + loc)) : 0u;
+        val[r] = ok ? idx_in[tile_base + loc] : 0u;
     }
     // warp-aggregated ranking: lanes with the same digit elect a leader that bumps the warp's counter
     const unsigned lt = (1u << lane) - 1;
@@ -305,6 +486,118 @@ k_radix_pass(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ 
     }
 }
 
+// ----------------------------------------------------------------------------- perm
+// cell_base[k] = new_off[k] + (#movers into k from below) - a_k + (#movers before position a_k),
+// so that the stayer at position i of cell k goes to cell_base[k] + i - (#movers before i).
+__global__ void __launch_bounds__(256) k_cell_base(const int32_t* __restrict__ new_off, const int32_t* __restrict__ old_off,
+                                                   const int32_t* __restrict__ mover_lo, const uint32_t* __restrict__ mask,
+                                                   const uint32_t* __restrict__ mprefix, int32_t* __restrict__ cell_base, int C,
+                                                   const uint32_t* __restrict__ counters)
+{
+    if (counters[kCtrHintBad]) return;                 // no stayers
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= C) return;
+    const int32_t a = old_off[k];
+    const uint32_t mv = mprefix[a >> 5] + __popc(mask[a >> 5] & ((1u << (a & 31)) - 1u));
+    cell_base[k] = new_off[k] + mover_lo[k] - a + (int32_t)mv;
+}
+
+// movers, sorted by (key, position): the r-th mover of key k goes below the stayers if it comes
+// from below the hint interval of k, else above them
+__global__ void __launch_bounds__(256) k_perm_movers(const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
+                                                     const int32_t* __restrict__ new_off, const int32_t* __restrict__ mover_off,
+                                                     const int32_t* __restrict__ old_off, int32_t* __restrict__ perm,
+                                                     const uint32_t* __restrict__ counters)
+{
+    const int64_t nm = counters[kCtrMovers];
+    const bool hint_ok = counters[kCtrHintBad] == 0u;
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < nm; q += (int64_t)gridDim.x * blockDim.x) {
+        const int k = (int)skey[q];
+        const int32_t i = (int32_t)sidx[q];
+        const int32_t m0 = mover_off[k], m1 = mover_off[k + 1];
+        const int32_t n0 = new_off[k], n1 = new_off[k + 1];
+        const int32_t stay = (n1 - n0) - (m1 - m0);
+        const bool below = hint_ok && i < old_off[k];
+        perm[n0 + ((int32_t)q - m0) + (below ? 0 : stay)] = i;
+    }
+}
+
+// stayers: position i (mover bit clear) belongs to the cell k whose hint interval holds i, i.e.
+// k = (first cell of the tile) + #{cells whose interval ends at or before i}; that count is a
+// prefix sum over the tile of "interval ends here" marks
+__global__ void __launch_bounds__(kClsThreads)
+k_perm_stayers(const int32_t* __restrict__ old_off, const int32_t* __restrict__ tile_first, const int32_t* __restrict__ cell_base,
+               const uint32_t* __restrict__ mask, const uint32_t* __restrict__ mprefix, int32_t* __restrict__ perm, int C,
+               int64_t n, const uint32_t* __restrict__ counters)
+{
+    if (counters[kCtrHintBad]) return;
+    __shared__ int s_ends[kClsTile];                     // number of intervals ending at each position -> home cell
+    __shared__ int s_warp[kClsWarps];
+    __shared__ int s_more;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t t0 = (int64_t)blockIdx.x * kClsTile;
+    const int64_t t1 = (t0 + kClsTile < n) ? t0 + kClsTile : n;
+    // anything to do?  (tiles made of movers only are common in the first, unsorted step)
+    bool any = false;
+    for (int64_t w = (t0 >> 5) + tid; w < ((t1 + 31) >> 5); w += kClsThreads) {
+        const int64_t left = t1 - (w << 5);
+        const uint32_t validbits = left >= 32 ? 0xFFFFFFFFu : ((1u << left) - 1u);
+        any = any || ((~mask[w]) & validbits) != 0u;
+    }
+    if (!__syncthreads_or(any)) return;
+
+    for (int i = tid; i < kClsTile; i += kClsThreads) s_ends[i] = 0;
+    __syncthreads();
+    const int c0 = tile_first[blockIdx.x];
+    for (int kb = c0;; kb += kClsThreads) {              // cells c0, c0+1, ... until an interval ends beyond the tile
+        const int k = kb + tid;
+        bool more = false;
+        if (k < C) {
+            const int64_t b = old_off[k + 1];
+            if (b < t1) {
+                if (b >= t0) atomicAdd(&s_ends[(int)(b - t0)], 1);
+                more = true;                                // intervals are ordered: later cells may still end inside
+            }
+        }
+        if (tid == kClsThreads - 1) s_more = (more && k + 1 < C) ? 1 : 0;
+        __syncthreads();
+        const int go = s_more;
+        __syncthreads();
+        if (!go) break;
+    }
+    // inclusive prefix sum of s_ends over the tile (blocked: 8 consecutive positions per thread)
+    int v[kClsIPT], sum = 0;
+#pragma unroll
+    for (int r = 0; r < kClsIPT; ++r) { sum += s_ends[tid * kClsIPT + r]; v[r] = sum; }
+    int inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    int off = c0 + inc - sum;
+    for (int w = 0; w < warp; ++w) off += s_warp[w];
+#pragma unroll
+    for (int r = 0; r < kClsIPT; ++r) s_ends[tid * kClsIPT + r] = off + v[r];
+    __syncthreads();
+    // coalesced over positions
+#pragma unroll
+    for (int r = 0; r < kClsIPT; ++r) {
+        const int loc = r * kClsThreads + tid;
+        const int64_t i = t0 + loc;
+        if (i < t1) {
+            const uint32_t m = mask[i >> 5];
+            if (!((m >> (i & 31)) & 1u)) {
+                const int k = s_ends[loc];
+                const uint32_t mv = mprefix[i >> 5] + __popc(m & ((1u << (i & 31)) - 1u));
+                perm[cell_base[k] + (int32_t)i - (int32_t)mv] = (int32_t)i;
+            }
+        }
+    }
+}
+
 // ----------------------------------------------------------------------------- reorder
 // a4: out_a[j] = in_a[perm[j]] for all attributes, bit for bit; coalesced writes, gathered reads.
 template <typename T, int D>
@@ -340,9 +633,11 @@ static int64_t cells_of(const pic_grid_t& g)
 }
 
 struct SortLayout {
-    size_t keys0, keys1, idx0, idx1, zero_begin, cell_count, digit_hist, scan_status, counters, lookback, zero_end, racc, total;
+    size_t keys0, keys1, idx0, idx1, mask, mprefix, old_off, mover_off, cell_base, tile_first, tile_count, tile_base, lookback;
+    size_t zero_begin, cell_count, mover_count, mover_lo, digit_hist, scan_status, cls_status, counters, zero_end;
+    size_t racc, total;
     int passes, bits, key_bits;
-    int64_t radix_tiles, scan_tiles;
+    int64_t radix_tiles, scan_tiles, cls_tiles;
 };
 
 static SortLayout sort_layout(const pic_grid_t& g, int64_t n)
@@ -354,18 +649,32 @@ static SortLayout sort_layout(const pic_grid_t& g, int64_t n)
     L.bits = (L.key_bits + L.passes - 1) / L.passes;
     L.radix_tiles = (n + kRadixTile - 1) / kRadixTile;
     L.scan_tiles = (C + kScanTile - 1) / kScanTile;
+    L.cls_tiles = (n + kClsTile - 1) / kClsTile;
     size_t off = 0;
     const size_t nb = align256(sizeof(uint32_t) * (size_t)(n > 0 ? n : 1));
+    const size_t wb = align256(sizeof(uint32_t) * (size_t)((n + 31) / 32 + 2));
+    const size_t cb = align256(sizeof(int32_t) * (size_t)(C + 1));
     L.keys0 = off; off += nb;
     L.keys1 = off; off += nb;
     L.idx0 = off; off += nb;
     L.idx1 = off; off += nb;
-    L.zero_begin = off;
-    L.cell_count = off; off += align256(sizeof(int32_t) * (size_t)C);
-    L.digit_hist = off; off += align256(sizeof(uint32_t) * kMaxPasses * kRadix);
-    L.scan_status = off; off += align256(sizeof(uint32_t) * (size_t)L.scan_tiles);
-    L.counters = off; off += 256;
+    L.mask = off; off += wb;
+    L.mprefix = off; off += wb;
+    L.old_off = off; off += cb;
+    L.mover_off = off; off += cb;
+    L.cell_base = off; off += cb;
+    L.tile_first = off; off += align256(sizeof(int32_t) * (size_t)(L.cls_tiles + 1));
+    L.tile_count = off; off += align256(sizeof(int32_t) * (size_t)(L.cls_tiles + 1));
+    L.tile_base = off; off += align256(sizeof(int32_t) * (size_t)(L.cls_tiles + 2));
     L.lookback = off; off += align256(sizeof(uint32_t) * (size_t)L.passes * (size_t)(L.radix_tiles > 0 ? L.radix_tiles : 1) * kRadix);
+    L.zero_begin = off;
+    L.cell_count = off; off += cb;
+    L.mover_count = off; off += cb;
+    L.mover_lo = off; off += cb;
+    L.digit_hist = off; off += align256(sizeof(uint32_t) * kMaxPasses * kRadix);
+    L.scan_status = off; off += align256(sizeof(uint32_t) * 2 * (size_t)L.scan_tiles);
+    L.cls_status = off; off += align256(sizeof(uint32_t) * (size_t)((L.cls_tiles + kScanTile - 1) / kScanTile + 1));
+    L.counters = off; off += 256;
     L.zero_end = off;
     L.racc = off; off += align256(sizeof(double) * (size_t)C);
     L.total = off;
@@ -383,11 +692,22 @@ int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, Sor
     o.keys[1] = (uint32_t*)(b + L.keys1);
     o.idx[0] = (uint32_t*)(b + L.idx0);
     o.idx[1] = (uint32_t*)(b + L.idx1);
+    o.mask = (uint32_t*)(b + L.mask);
+    o.mprefix = (uint32_t*)(b + L.mprefix);
+    o.old_off = (int32_t*)(b + L.old_off);
+    o.mover_off = (int32_t*)(b + L.mover_off);
+    o.cell_base = (int32_t*)(b + L.cell_base);
+    o.tile_first = (int32_t*)(b + L.tile_first);
+    o.tile_count = (int32_t*)(b + L.tile_count);
+    o.tile_base = (int32_t*)(b + L.tile_base);
+    o.lookback = (uint32_t*)(b + L.lookback);
     o.cell_count = (int32_t*)(b + L.cell_count);
+    o.mover_count = (int32_t*)(b + L.mover_count);
+    o.mover_lo = (int32_t*)(b + L.mover_lo);
     o.digit_hist = (uint32_t*)(b + L.digit_hist);
     o.scan_status = (uint32_t*)(b + L.scan_status);
+    o.cls_status = (uint32_t*)(b + L.cls_status);
     o.counters = (uint32_t*)(b + L.counters);
-    o.lookback = (uint32_t*)(b + L.lookback);
     o.zero_begin = b + L.zero_begin;
     o.zero_bytes = L.zero_end - L.zero_begin;
     o.racc = (double*)(b + L.racc);
@@ -396,6 +716,7 @@ int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, Sor
     o.key_bits = L.key_bits;
     o.radix_tiles = L.radix_tiles;
     o.scan_tiles = L.scan_tiles;
+    o.cls_tiles = L.cls_tiles;
     return PIC_OK;
 }
 
@@ -407,35 +728,55 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
     const int C = (int)cells_of(g);
     mark_phase(PIC_PHASE_BEGIN, st);
     PIC_CUDA_OK(cudaMemsetAsync(ws.zero_begin, 0, ws.zero_bytes, st));
+    // the hint: cell_offsets as found on entry
+    k_hint_check<<<(unsigned)((C + 1 + 255) / 256), 256, 0, st>>>(cell_offsets, ws.old_off, C, n, ws.counters);
+    count_launch();
     if (n > 0) {
-        int blocks = (int)std::min<int64_t>((n + 255) / 256, 148 * 8);
-        k_keys_hist<T, D><<<blocks, 256, 0, st>>>(make_partp<T>(in), make_gridp<T>(g), n, ws.keys[0], ws.cell_count);
-        count_launch();
+        k_hint_tiles<<<(unsigned)((C + 1 + 255) / 256), 256, 0, st>>>(ws.old_off, C, (int)ws.cls_tiles, ws.tile_first, ws.counters);
+        // movers are staged per tile in the second halves of the ping-pong arrays, then packed
+        k_classify<T, D><<<(unsigned)ws.cls_tiles, kClsThreads, 0, st>>>(
+            make_partp<T>(in), make_gridp<T>(g), n, ws.old_off, ws.cell_count, ws.mover_count, ws.mover_lo, ws.keys[1],
+            ws.idx[1], ws.mask, ws.mprefix, ws.tile_count, ws.counters);
+        k_scan_cells<<<(unsigned)((ws.cls_tiles + kScanTile - 1) / kScanTile), kScanThreads, 0, st>>>(
+            ws.tile_count, ws.tile_base, (int)ws.cls_tiles, ws.cls_status, ws.counters + kCtrCls, nullptr, 0, 0);
+        k_movers_place<<<(unsigned)ws.cls_tiles, kClsThreads, 0, st>>>(ws.keys[1], ws.idx[1], ws.keys[0], ws.idx[0], ws.mask,
+                                                                      ws.mprefix, ws.tile_base, (int)ws.cls_tiles, n, ws.counters);
+        count_launch(4);
     }
     mark_phase(PIC_PHASE_KEYS, st);
     k_scan_cells<<<(unsigned)ws.scan_tiles, kScanThreads, 0, st>>>(ws.cell_count, cell_offsets, C, ws.scan_status,
-                                                                    ws.counters + 0, ws.digit_hist, ws.passes,
-                                                                    ws.bits_per_pass);
+                                                                    ws.counters + kCtrScanA, nullptr, 0, 0);
     count_launch();
     if (n > 0) {
+        k_scan_cells<<<(unsigned)ws.scan_tiles, kScanThreads, 0, st>>>(ws.mover_count, ws.mover_off, C,
+                                                                        ws.scan_status + ws.scan_tiles, ws.counters + kCtrScanB,
+                                                                        ws.digit_hist, ws.passes, ws.bits_per_pass);
         k_scan_digits<<<ws.passes, kRadix, 0, st>>>(ws.digit_hist);
-        count_launch();
+        const int64_t pass_stride = ws.radix_tiles * kRadix;
+        k_zero_lookback<<<148 * 4, 256, 0, st>>>(ws.lookback, ws.counters, ws.passes, pass_stride);
+        count_launch(3);
         mark_phase(PIC_PHASE_SCAN, st);
         int src = 0;
         for (int q = 0; q < ws.passes; ++q) {
             const bool last = q == ws.passes - 1;
-            const uint32_t* kin = ws.keys[src];
-            const uint32_t* iin = q == 0 ? nullptr : ws.idx[src];
-            uint32_t* kout = last ? nullptr : ws.keys[src ^ 1];
-            uint32_t* iout = last ? (uint32_t*)perm : ws.idx[src ^ 1];
             k_radix_pass<<<(unsigned)ws.radix_tiles, kRadixThreads, 0, st>>>(
-                kin, iin, kout, iout, n, q * ws.bits_per_pass, (1u << ws.bits_per_pass) - 1u, ws.digit_hist + q * kRadix, ws.counters + 1 + q,
-                ws.lookback + (size_t)q * (size_t)ws.radix_tiles * kRadix);
+                ws.keys[src], ws.idx[src], ws.keys[src ^ 1], ws.idx[src ^ 1], ws.counters, q * ws.bits_per_pass,
+                (1u << ws.bits_per_pass) - 1u, ws.digit_hist + q * kRadix, ws.counters + kCtrRadix + q,
+                ws.lookback + (size_t)q * (size_t)pass_stride);
+            (void)last;
             count_launch();
             src ^= 1;
         }
+        mark_phase(PIC_PHASE_RADIX, st);
+        k_cell_base<<<(unsigned)((C + 255) / 256), 256, 0, st>>>(cell_offsets, ws.old_off, ws.mover_lo, ws.mask, ws.mprefix,
+                                                                 ws.cell_base, C, ws.counters);
+        k_perm_movers<<<148 * 8, 256, 0, st>>>(ws.keys[src], ws.idx[src], cell_offsets, ws.mover_off, ws.old_off, perm,
+                                              ws.counters);
+        k_perm_stayers<<<(unsigned)ws.cls_tiles, kClsThreads, 0, st>>>(ws.old_off, ws.tile_first, ws.cell_base, ws.mask,
+                                                                      ws.mprefix, perm, C, n, ws.counters);
+        count_launch(3);
     }
-    mark_phase(PIC_PHASE_RADIX, st);
+    mark_phase(PIC_PHASE_REORDER, st);
     return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
 
@@ -450,7 +791,6 @@ static int sort_impl(const pic_grid_t& g, const pic_particles_t& in, pic_particl
         k_reorder<T, D><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(make_partp<T>(in), make_partp<T>(out), perm, n);
         count_launch();
     }
-    mark_phase(PIC_PHASE_REORDER, st);
     return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
 

@@ -44,7 +44,7 @@ constexpr int kG = 8;                  // lanes per item
 
 template <typename T>
 struct TileShape {
-    static constexpr int kTile = sizeof(T) == 4 ? 2048 : 1024;   // particles per block
+    static constexpr int kTile = sizeof(T) == 4 ? 1792 : 1024;   // particles per block (3 resident blocks of fp32)
     static constexpr int NB = sizeof(T) == 4 ? 2 : 1;            // particles per lane and batch
 };
 
@@ -255,11 +255,12 @@ struct TileSmem {
     static constexpr int kMaxItems = kTile + kTile / kItemMax + 2;
     static constexpr size_t part_bytes = sizeof(T) * A * kTile;
     static constexpr size_t field_bytes = sizeof(T) * GROUPS * ESTRIDE;
-    static constexpr size_t item_bytes = sizeof(uint32_t) * kMaxItems;
-    static constexpr size_t stray_bytes = sizeof(uint16_t) * kTile;
+    static constexpr size_t item_bytes = sizeof(uint32_t) * kMaxItems;               // (start, len) per item
+    static constexpr size_t order_bytes = (sizeof(uint16_t) * kMaxItems + 15) / 16 * 16;  // items, longest first
+    static constexpr size_t stray_bytes = sizeof(uint32_t) * (kTile / 32);          // one bit per slot
     static constexpr size_t bytes(int mode)
     {
-        return part_bytes + ((mode & kModePush) ? field_bytes : 0) + item_bytes + stray_bytes;
+        return part_bytes + ((mode & kModePush) ? field_bytes : 0) + item_bytes + order_bytes + stray_bytes;
     }
 };
 
@@ -267,7 +268,7 @@ template <typename T, int D, int P, int MODE>
 constexpr int tile_min_blocks()
 {
     // resident blocks per SM the kernel is compiled for (register budget 65536 / (128 * blocks))
-    return (sizeof(T) == 4) ? 2 : 1;
+    return (sizeof(T) == 4) ? 3 : 1;
 }
 
 template <typename T, int D, int P, int MODE, bool VIA_PERM>
@@ -295,10 +296,12 @@ k_tile(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
     T* const sp = reinterpret_cast<T*>(s_dyn);                                        // [A][kTile]
     T* const sE = reinterpret_cast<T*>(s_dyn + SM::part_bytes);                       // [GROUPS][ESTRIDE]
     uint32_t* const s_item = reinterpret_cast<uint32_t*>(s_dyn + SM::part_bytes + (PUSH ? SM::field_bytes : 0));
-    uint16_t* const s_stray = reinterpret_cast<uint16_t*>(reinterpret_cast<unsigned char*>(s_item) + SM::item_bytes);
-    __shared__ int s_scan[kTileThreads / 32];
+    uint16_t* const s_order = reinterpret_cast<uint16_t*>(reinterpret_cast<unsigned char*>(s_item) + SM::item_bytes);
+    uint32_t* const s_stray = reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned char*>(s_order) + SM::order_bytes);
+    constexpr int kClasses = 16;                // items are queued by number of batches, longest first
+    __shared__ int s_cls[kClasses + 1];
     __shared__ int s_cells[2];
-    __shared__ int s_nitems, s_next, s_nstray;
+    __shared__ int s_nitems, s_next, s_anystray;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lg = lane % G;                    // lane within the group
@@ -310,26 +313,38 @@ k_tile(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
     //         Row a of the staged tile: x[a] for a < D, v[a-D] for a < 2D, w for a == 2D.
     auto needed = [](int a) { return a < D || (a < 2 * D ? (PUSH || VIA_PERM) : (DEP || VIA_PERM)); };
     auto src_row = [&](int a) -> const T* { return a < D ? src.x[a] : (a < 2 * D ? src.v[a - D] : src.w); };
-    for (int q = tid * VEC; q < cnt; q += kTileThreads * VEC) {
-        if (q + VEC <= cnt) {
-            T val[A][VEC];
-            if constexpr (VIA_PERM) {
-                int idx[VEC];
-                if constexpr (VEC == 4) {
-                    const int4 p4 = *reinterpret_cast<const int4*>(perm + j0 + q);
-                    idx[0] = p4.x; idx[1] = p4.y; idx[2] = p4.z; idx[3] = p4.w;
-                } else {
-                    const int2 p2 = *reinterpret_cast<const int2*>(perm + j0 + q);
-                    idx[0] = p2.x; idx[1] = p2.y;
-                }
+    if constexpr (VIA_PERM) {
+        // consecutive lanes take consecutive slots: particles that kept their cell sit in runs of
+        // consecutive source indices, so most of a warp's 32 loads fall into one or two lines
+        constexpr int U = 4;                    // slots per thread in flight (U perm words, then U*A loads)
+        for (int q0 = 0; q0 < cnt; q0 += kTileThreads * U) {
+            int idx[U];
 #pragma unroll
-                for (int a = 0; a < A; ++a) {
-                    if (!needed(a)) continue;
-                    const T* arr = src_row(a);
+            for (int u = 0; u < U; ++u) {
+                const int q = q0 + u * kTileThreads + tid;
+                idx[u] = q < cnt ? perm[j0 + q] : -1;
+            }
+            T val[A][U];
 #pragma unroll
-                    for (int e = 0; e < VEC; ++e) val[a][e] = arr[idx[e]];
-                }
-            } else {
+            for (int a = 0; a < A; ++a) {
+                if (!needed(a)) continue;
+                const T* arr = src_row(a);
+#pragma unroll
+                for (int u = 0; u < U; ++u)
+                    if (idx[u] >= 0) val[a][u] = arr[idx[u]];
+            }
+#pragma unroll
+            for (int a = 0; a < A; ++a) {
+                if (!needed(a)) continue;
+#pragma unroll
+                for (int u = 0; u < U; ++u)
+                    if (idx[u] >= 0) sp[a * kTile + q0 + u * kTileThreads + tid] = val[a][u];
+            }
+        }
+    } else {
+        for (int q = tid * VEC; q < cnt; q += kTileThreads * VEC) {
+            if (q + VEC <= cnt) {
+                T val[A][VEC];
 #pragma unroll
                 for (int a = 0; a < A; ++a) {
                     if (!needed(a)) continue;
@@ -342,25 +357,26 @@ k_tile(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
                         val[a][0] = v2.x; val[a][1] = v2.y;
                     }
                 }
-            }
 #pragma unroll
-            for (int a = 0; a < A; ++a) {
-                if (!needed(a)) continue;
-                if constexpr (VEC == 4)
-                    *reinterpret_cast<float4*>(sp + a * kTile + q) = make_float4(val[a][0], val[a][1], val[a][2], val[a][3]);
-                else
-                    *reinterpret_cast<double2*>(sp + a * kTile + q) = make_double2(val[a][0], val[a][1]);
-            }
-        } else {
-            for (int e = 0; q + e < cnt; ++e) {
-                const int64_t i = VIA_PERM ? (int64_t)perm[j0 + q + e] : j0 + q + e;
+                for (int a = 0; a < A; ++a) {
+                    if (!needed(a)) continue;
+                    if constexpr (VEC == 4)
+                        *reinterpret_cast<float4*>(sp + a * kTile + q) = make_float4(val[a][0], val[a][1], val[a][2], val[a][3]);
+                    else
+                        *reinterpret_cast<double2*>(sp + a * kTile + q) = make_double2(val[a][0], val[a][1]);
+                }
+            } else {
+                for (int e = 0; q + e < cnt; ++e) {
 #pragma unroll
-                for (int a = 0; a < A; ++a)
-                    if (needed(a)) sp[a * kTile + q + e] = src_row(a)[i];
+                    for (int a = 0; a < A; ++a)
+                        if (needed(a)) sp[a * kTile + q + e] = src_row(a)[j0 + q + e];
+                }
             }
         }
     }
-    if (tid == 0) { s_nitems = 0; s_next = 0; s_nstray = 0; }
+    for (int i = tid; i < kTile / 32; i += kTileThreads) s_stray[i] = 0u;
+    if (tid <= kClasses) s_cls[tid] = 0;
+    if (tid == 0) { s_nitems = 0; s_next = 0; s_anystray = 0; }
     __syncthreads();
 
     // ---- 2. cells whose runs (by cell_offsets) hold the first and the last slot of the tile: the key
@@ -390,37 +406,36 @@ k_tile(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
     {
         const int c_first = s_cells[0], c_last = s_cells[1];
         const int64_t j1 = j0 + cnt;
-        for (int base = c_first; base <= c_last; base += kTileThreads) {
-            const int c = base + tid;
-            int s = 0, len = 0;
-            if (c <= c_last) {
-                const int64_t a = cell_offsets[c], b = cell_offsets[c + 1];
-                const int64_t lo = a > j0 ? a : j0, hi = b < j1 ? b : j1;
-                s = (int)(lo - j0);
-                len = hi > lo ? (int)(hi - lo) : 0;
-            }
+        for (int c = c_first + tid; c <= c_last; c += kTileThreads) {
+            const int64_t a = cell_offsets[c], b = cell_offsets[c + 1];
+            const int64_t lo = a > j0 ? a : j0, hi = b < j1 ? b : j1;
+            const int s = (int)(lo - j0);
+            const int len = hi > lo ? (int)(hi - lo) : 0;
             const int nch = (len + kItemMax - 1) / kItemMax;
-            int inc = nch;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                int t = __shfl_up_sync(FULL, inc, o);
-                if (lane >= o) inc += t;
-            }
-            if (lane == 31) s_scan[warp] = inc;
-            __syncthreads();
-            int off = s_nitems;
-            for (int w = 0; w < warp; ++w) off += s_scan[w];
-            const int pos = off + inc - nch;
-            for (int q = 0; q < nch; ++q) {
-                if (pos + q < SM::kMaxItems) {
-                    const int rem = len - q * kItemMax;
-                    s_item[pos + q] = (uint32_t)(s + q * kItemMax) | ((uint32_t)(rem < kItemMax ? rem : kItemMax) << 16);
+            if (nch > 0) {
+                const int pos = atomicAdd(&s_nitems, nch);
+                for (int q = 0; q < nch; ++q) {
+                    if (pos + q < SM::kMaxItems) {
+                        const int rem = len - q * kItemMax;
+                        const int l = rem < kItemMax ? rem : kItemMax;
+                        s_item[pos + q] = (uint32_t)(s + q * kItemMax) | ((uint32_t)l << 16);
+                        atomicAdd(&s_cls[kClasses - (l + G * NB - 1) / (G * NB)], 1);   // class 0 = longest
+                    }
                 }
             }
-            __syncthreads();
-            if (tid == kTileThreads - 1) s_nitems = (off + inc < SM::kMaxItems) ? off + inc : SM::kMaxItems;
-            __syncthreads();
         }
+        __syncthreads();
+        if (tid == 0) {                         // exclusive prefix over the classes
+            int run = 0;
+            for (int k = 0; k <= kClasses; ++k) { const int c = s_cls[k]; s_cls[k] = run; run += c; }
+            if (s_nitems > SM::kMaxItems) s_nitems = SM::kMaxItems;
+        }
+        __syncthreads();
+        for (int i = tid; i < s_nitems; i += kTileThreads) {
+            const int l = (int)(s_item[i] >> 16);
+            s_order[atomicAdd(&s_cls[kClasses - (l + G * NB - 1) / (G * NB)], 1)] = (uint16_t)i;
+        }
+        __syncthreads();
     }
     const int nitems = s_nitems;
     T* const myE = sE + gid * SM::ESTRIDE;
@@ -433,7 +448,7 @@ k_tile(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
         if (ibase >= nitems) break;
         const int item = ibase + lane / G;
         const bool have = item < nitems;
-        const uint32_t it = have ? s_item[item] : 0u;
+        const uint32_t it = have ? s_item[s_order[item]] : 0u;
         const int start = (int)(it & 0xFFFFu), len = (int)(it >> 16);
 
         // the item's cell, from its first particle
@@ -496,7 +511,7 @@ k_tile(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
                 } else {
                     wz[b][0] = (T)1;
                 }
-                if (in_item && !same) s_stray[atomicAdd(&s_nstray, 1)] = (uint16_t)slot[b];
+                if (in_item && !same) { atomicOr(&s_stray[slot[b] >> 5], 1u << (slot[b] & 31)); s_anystray = 1; }
                 live[b] = in_item && same;
                 q[b] = (T)0;
                 if constexpr (DEP) {
@@ -580,11 +595,10 @@ k_tile(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
     __syncthreads();
 
     // ---- 4. particles whose cell is not their run's cell (only with inconsistent cell_offsets)
-    {
-        const int ns = s_nstray;
-        for (int i = tid; i < ns; i += kTileThreads)
-            stray_particle<T, D, P, MODE>(sp, kTile, (int)s_stray[i], g, f, racc, dt, qmdt);
-        if (ns > 0) __syncthreads();
+    if (s_anystray) {
+        for (int i = tid; i < cnt; i += kTileThreads)
+            if ((s_stray[i >> 5] >> (i & 31)) & 1u) stray_particle<T, D, P, MODE>(sp, kTile, i, g, f, racc, dt, qmdt);
+        __syncthreads();
     }
 
     // ---- 5. write the tile back (x, v; w too when the reorder is fused in)

@@ -112,6 +112,62 @@ def test_sort_degenerate_inputs():
         assert np.array_equal(off.cpu().numpy(), ro[4])
 
 
+def _gpu_sort_hint(B, g, x, v, w, hint):
+    """pic_sort with cell_offsets pre-filled with `hint` (the library reads it as the order hint)."""
+    n = w.shape[0]
+    xd, vd, wd = to_dev(x), to_dev(v), to_dev([w])[0]
+    xo = [torch.empty_like(a) for a in xd]
+    vo = [torch.empty_like(a) for a in vd]
+    wo = torch.empty_like(wd)
+    perm = torch.full((max(n, 4),), -1, dtype=torch.int32, device="cuda")
+    off = torch.from_numpy(np.concatenate([hint.astype(np.int32), np.zeros(3, np.int32)])).cuda()
+    ws = torch.empty(B.pic_workspace_bytes(g, n), dtype=torch.uint8, device="cuda")
+    B.pic_sort(g, xd, vd, wd, xo, vo, wo, perm, off, ws)
+    torch.cuda.synchronize()
+    return perm[:n].cpu().numpy(), off[: g.cells + 1].cpu().numpy(), xo
+
+
+@pytest.mark.parametrize("name,kw", [
+    ("cfg2", dict(N=200_003, n=(64, 64))),
+    ("cfg3", dict(N=150_001, n=(32, 32, 32))),
+    ("cfg4", dict(N=300_007, n=(32, 32, 32))),
+    ("cfg5", dict(N=8 * 16 ** 3 + 5, n=(16, 16, 16))),
+    ("cfg3", dict(N=5_000, n=(32, 32, 32))),          # far fewer particles than cells: long runs of empty cells
+])
+def test_sort_with_order_hint(name, kw):
+    """Whatever cell_offsets holds on entry, the result is the unique stable permutation (R7)."""
+    O, B = _mods()
+    cfg = _cfg(name, kw)
+    wl = W.make_workload(cfg)
+    go, gb = O.grid_of(cfg), B.grid_of(cfg)
+    r1 = O.step(go, wl.x, wl.v, wl.w, wl.E, cfg.dt, cfg.qm)            # sorted at t, pushed to t+1
+    r2 = O.step(go, r1["x"], r1["v"], r1["w"], wl.E, cfg.dt, cfg.qm)    # sorted at t+1, pushed to t+2
+    x, v, w = r2["x"], r2["v"], r2["w"]                                # order = cells at t+1
+    ref = O.sort(go, x, v, w)
+    C, n = gb.cells, cfg.N
+    rng = np.random.default_rng(5)
+    hints = {
+        "previous offsets (steady state)": r2["cell_offsets"],
+        "offsets of two steps ago": r1["cell_offsets"],
+        "the new offsets themselves": ref[4],
+        "all zero": np.zeros(C + 1, np.int64),
+        "all N": np.full(C + 1, n, np.int64),
+        "random non-decreasing": np.sort(rng.integers(0, n + 1, C + 1)),
+        "random, not monotone": rng.integers(0, n + 1, C + 1),
+        "out of range": np.arange(C + 1, dtype=np.int64) * 7 - 3,
+        "one interval holds everything": np.concatenate([np.zeros(C // 2 + 1, np.int64), np.full(C - C // 2, n, np.int64)]),
+    }
+    for what, hint in hints.items():
+        perm, off, xo = _gpu_sort_hint(B, gb, x, v, w, np.asarray(hint))
+        assert np.array_equal(off, ref[4]), what
+        assert np.array_equal(perm, ref[3]), what
+        assert np.array_equal(xo[0].cpu().numpy(), ref[0][0]), what
+    # an input that is already sorted, with its own offsets as the hint: identity
+    xs, vs, wsrt, _, offs = ref
+    perm, off, _ = _gpu_sort_hint(B, gb, xs, vs, wsrt, offs)
+    assert np.array_equal(perm, np.arange(n, dtype=np.int32)) and np.array_equal(off, offs)
+
+
 @pytest.mark.parametrize("order", ORDERS)
 @pytest.mark.parametrize("name,kw", SMALL)
 def test_deposit_parity(name, kw, order):
