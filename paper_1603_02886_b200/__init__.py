@@ -25,12 +25,15 @@ EXPORTS = ("pic_workspace_bytes", "pic_sort", "pic_deposit", "pic_push", "pic_st
 PHASES = ("begin", "keys", "scan", "radix", "reorder", "deposit", "push")
 
 # True once pic_step runs deposit + gather + push as ONE kernel (recorded as phase "push")
-FUSED_PHASE_IS_PUSH = False
+FUSED_PHASE_IS_PUSH = True
 
 
 def fused_kernel_bytes(dim: int, itemsize: int, with_sort: bool) -> int:
-    """Algorithmic bytes per particle of the fused deposit+push kernel: read x, v, w; write x, v."""
-    return (4 * dim + 1) * itemsize
+    """Algorithmic bytes per particle of the fused kernel: read x, v, w and write x, v (in place), or,
+    with the sort's reorder fused in, read all A = 2d+1 attributes and write all of them to `out`.
+    perm (an integer side array) is overhead and is not counted ("Byte model")."""
+    a = 2 * dim + 1
+    return (2 * a if with_sort else a + 2 * dim) * itemsize
 
 
 class PicError(RuntimeError):

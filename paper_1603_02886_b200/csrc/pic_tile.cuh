@@ -39,12 +39,15 @@ struct FieldP {
 
 enum { kModeDeposit = 1, kModePush = 2, kModeBoth = 3 };
 
-constexpr int kTileThreads = 128;
+#ifndef PIC_TILE_THREADS
+#define PIC_TILE_THREADS 128
+#endif
+constexpr int kTileThreads = PIC_TILE_THREADS;
 constexpr int kG = 8;                  // lanes per item
 
 template <typename T>
 struct TileShape {
-    static constexpr int kTile = sizeof(T) == 4 ? 1792 : 1024;   // particles per block (3 resident blocks of fp32)
+    static constexpr int kTile = (sizeof(T) == 4 ? 1792 : 1024) * kTileThreads / 128;   // particles per block (3 resident blocks of fp32)
     static constexpr int NB = sizeof(T) == 4 ? 2 : 1;            // particles per lane and batch
 };
 
@@ -268,7 +271,7 @@ template <typename T, int D, int P, int MODE>
 constexpr int tile_min_blocks()
 {
     // resident blocks per SM the kernel is compiled for (register budget 65536 / (128 * blocks))
-    return (sizeof(T) == 4) ? 3 : 1;
+    return ((sizeof(T) == 4) ? 3 : 1) * (128 / kTileThreads);
 }
 
 template <typename T, int D, int P, int MODE, bool VIA_PERM>
