@@ -12,7 +12,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpic_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+         "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("PIC_NVCC_EXTRA", "").split()
 
 
 def sources():
