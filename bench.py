@@ -159,6 +159,21 @@ def workload_config(cfg, args, sample=None):
             "timed": "steady state after warm-up steps that include the first random-order sort"}
 
 
+def max_over_ranks(value, dist, device):
+    """Max of a per-rank scalar over all ranks (the timing rule: max over ranks); identity without dist."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_throughput(n_per_rank, world, steps, ms_total_max):
+    """Replicas only: every rank advances its own n_per_rank particles; value = all particle-steps / max time."""
+    return n_per_rank * world * steps / (ms_total_max * 1e-3)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -251,12 +266,9 @@ def main():
     barrier()
     clocks = sampler.stop()
     ms_total = t_begin.elapsed_time(t_end)
-    if world > 1:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dist if world > 1 else None, dev)
     ms_step = ms_total / K
-    value = cfg.N * world * K / (ms_total * 1e-3)
+    value = replica_throughput(cfg.N, world, K, ms_total)
 
     # ---- per-phase durations from the events recorded inside the timed region
     phases = {}
@@ -346,10 +358,7 @@ def run_e2e(B, torch, cfg, g, wl, dev, K, world, dist):
         cur, nxt = nxt, cur
     torch.cuda.synchronize()
     el = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([el], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        el = float(t.item())
+    el = max_over_ranks(el, dist, dev)
     return {"value": n * world * steps / el, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
             "steps": steps, "ms_per_step": 1e3 * el / steps,
             "api": "pic_step_host (pinned host buffers, sort every step)"}

@@ -420,7 +420,11 @@ k_rows(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
 
         // ---- end of the item: this lane's node sums go to the grid
         if constexpr (DEP) {
+#ifdef PIC_EXP_NORED
+            if (have && acc[0][0].r == 0x123456789abcdefull) {
+#else
             if (have) {
+#endif
 #pragma unroll
                 for (int rr = 0; rr < RPL; ++rr)
 #pragma unroll
