@@ -60,14 +60,13 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/r01_v3_rows.md): key = "<config>:<phase of the dominant kernel>"
+NCU_TRAFFIC = {"cfg3:push": 8.32e9}
+
+
 def ncu_traffic(cfg_name, kernel):
-    """dram bytes read+written per launch of the dominant kernel, from the committed ncu capture
-    (profiles/ncu_traffic.json, written by hand from `ncu --set full`); None if not captured."""
-    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
-    try:
-        return json.load(open(p)).get("%s:%s" % (cfg_name, kernel))
-    except Exception:
-        return None
+    return NCU_TRAFFIC.get("%s:%s" % (cfg_name, kernel))
 
 
 class ClockSampler:
