@@ -151,12 +151,12 @@ void mark_phase(int phase, cudaStream_t st);
 struct SortWs {
     uint32_t* keys[2];       // [N] movers' keys, ping-pong
     uint32_t* idx[2];        // [N] movers' positions, ping-pong
+    uint32_t* pkey;          // [N] key of every position
     uint32_t* mask;          // [N/32 + 2] mover bit of every position
     uint32_t* mprefix;       // [N/32 + 2] movers before each 32-position word
     int32_t* old_off;        // [C+1] the hint: cell_offsets as found on entry
     int32_t* mover_off;      // [C+1] exclusive scan of mover_count
     int32_t* cell_base;      // [C]   where the stayers of a cell start in perm (see k_cell_base)
-    int32_t* tile_first;     // [classify tiles] first cell of every classify tile
     int32_t* tile_count;     // [classify tiles] movers per tile
     int32_t* tile_base;      // [classify tiles + 1] exclusive scan of tile_count
     uint32_t* lookback;      // [passes][radix tiles][kRadix]

@@ -22,7 +22,6 @@
 //     its scan place each mover inside its cell.
 //
 // Kernels:  k_hint_check     hint -> private copy, validity flag
-//           k_hint_tiles     first cell of every 4096-position tile (for k_perm_stayers)
 //           k_classify       x[d] -> key, histograms, stayer/mover split, movers compacted in order
 //           k_scan_cells     count[C] -> exclusive offsets [C+1] (single pass, decoupled look-back)
 //           k_scan_digits    digit histograms -> exclusive global digit offsets
@@ -106,95 +105,71 @@ __global__ void __launch_bounds__(256) k_hint_check(const int32_t* __restrict__ 
     if (bad) counters[kCtrHintBad] = 1u;
 }
 
-// tile_first[t] = smallest k with old_off[k+1] > t*kClsTile (C if none): the first cell whose
-// interval can hold a position of tile t.  One thread per cell; the loop lengths add up to
-// (#tiles + C) because the hint is non-decreasing (the kernel does nothing for a bad hint).
-__global__ void __launch_bounds__(256) k_hint_tiles(const int32_t* __restrict__ old_off, int C, int ntiles,
-                                                    int32_t* __restrict__ tile_first, const uint32_t* __restrict__ counters)
-{
-    if (counters[kCtrHintBad]) return;
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k > C) return;
-    // tiles t with b_{k-1} <= t*kClsTile < b_k, where b_k = old_off[k+1], b_{-1} = 0, b_C = +inf
-    const int64_t lo = k == 0 ? 0 : old_off[k];
-    const int64_t hi = k == C ? (int64_t)ntiles * kClsTile : old_off[k + 1];
-    for (int64_t t = (lo + kClsTile - 1) / kClsTile; t * kClsTile < hi && t < ntiles; ++t) tile_first[t] = k;
-}
-
 // ----------------------------------------------------------------------------- keys, histograms, stayer/mover split
 // a1: key = c_x + n_x*(c_y + n_y*c_z) (x fastest), clamped cell index
 // (PAPER.md:493-497).  a2: count[key]++ -- consecutive lanes holding the same key (the common
 // case once the particles are pre-ordered) are merged into one atomic per run.
 // Movers (see the header) are appended to (mkey, midx) in position order; mask / mprefix hold,
 // per 32 positions, the movers' bits and the number of movers before the word.
-template <typename T, int D>
-__global__ void __launch_bounds__(kClsThreads)
-k_classify(PartP<T> p, GridP<T> g, int64_t n, const int32_t* __restrict__ old_off, int32_t* __restrict__ cell_count,
-           int32_t* __restrict__ mover_count, int32_t* __restrict__ mover_lo, uint32_t* __restrict__ mkey,
-           uint32_t* __restrict__ midx, uint32_t* __restrict__ mask, uint32_t* __restrict__ mprefix,
-           int32_t* __restrict__ tile_count, const uint32_t* __restrict__ counters)
+// One warp's 32*kClsIPT positions.  CHECK = false: all of them are below n (no bounds tests).
+template <typename T, int D, bool CHECK>
+__device__ __forceinline__ void classify_warp(const PartP<T>& p, const GridP<T>& g, int n, int wbase, unsigned lane, bool hint_ok,
+                                              const int32_t* __restrict__ old_off, int32_t* __restrict__ cell_count,
+                                              uint32_t* __restrict__ pkey, uint32_t (&key)[kClsIPT], uint32_t (&bal)[kClsIPT],
+                                              uint32_t& mover_bits, uint32_t& lo_bits)
 {
-    __shared__ uint32_t s_wsum[kClsWarps];
-    const unsigned tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int tile = (int)blockIdx.x;
-    const bool hint_ok = counters[kCtrHintBad] == 0u;
-    const int64_t wbase = (int64_t)tile * kClsTile + warp * (32 * kClsIPT);
-
+    const int i0 = wbase + (int)lane;
     // all positions of this thread first: independent loads
     T xs[D][kClsIPT];
 #pragma unroll
-    for (int r = 0; r < kClsIPT; ++r) {
-        const int64_t i = wbase + r * 32 + lane;
+    for (int c = 0; c < D; ++c) {
+        const T* __restrict__ xc = p.x[c] + i0;
 #pragma unroll
-        for (int c = 0; c < D; ++c) xs[c][r] = i < n ? p.x[c][i] : (T)0;
+        for (int r = 0; r < kClsIPT; ++r) xs[c][r] = (!CHECK || i0 + r * 32 < n) ? xc[r * 32] : (T)0;
     }
-    uint32_t key[kClsIPT], bal[kClsIPT];
-    uint32_t mover_bits = 0, lo_bits = 0;
 #pragma unroll
     for (int r = 0; r < kClsIPT; ++r) {
-        const int64_t i = wbase + r * 32 + lane;
-        key[r] = 0xFFFFFFFFu;
-        if (i < n) {
-            int k = 0, mul = 1;
+        int k = 0, mul = 1;
 #pragma unroll
-            for (int c = 0; c < D; ++c) {
-                T t = grid_coord(xs[c][r], g.h[c], g.inv_h[c], g.hmul);
-                k += mul * cell_index(t, g.n[c]);
-                mul *= g.n[c];
-            }
-            key[r] = (uint32_t)k;
+        for (int c = 0; c < D; ++c) {
+            T t = grid_coord(xs[c][r], g.h[c], g.inv_h[c], g.hmul);
+            k += mul * cell_index(t, g.n[c]);
+            mul *= g.n[c];
         }
+        key[r] = (!CHECK || i0 + r * 32 < n) ? (uint32_t)k : 0xFFFFFFFFu;
+        if (!CHECK || i0 + r * 32 < n) pkey[i0 + r * 32] = (uint32_t)k;
     }
-    // the hint intervals of the new keys: independent loads again
+    // the hint intervals of the new keys: independent loads again.  stayer <=> ha <= i < hb
+    mover_bits = 0;
+    lo_bits = 0;
     if (hint_ok) {
         int32_t ha[kClsIPT], hb[kClsIPT];
 #pragma unroll
         for (int r = 0; r < kClsIPT; ++r) {
-            const bool valid = key[r] != 0xFFFFFFFFu;
+            const bool valid = !CHECK || key[r] != 0xFFFFFFFFu;
             ha[r] = valid ? old_off[key[r]] : 0;
             hb[r] = valid ? old_off[key[r] + 1] : 0;
         }
 #pragma unroll
         for (int r = 0; r < kClsIPT; ++r) {
-            const int64_t i = wbase + r * 32 + lane;
-            if (key[r] != 0xFFFFFFFFu) {
-                if (!((int64_t)ha[r] <= i && i < (int64_t)hb[r])) mover_bits |= 1u << r;
-                if (i < (int64_t)ha[r]) lo_bits |= 1u << r;
-            }
+            const int i = i0 + r * 32;
+            const bool valid = !CHECK || key[r] != 0xFFFFFFFFu;
+            const bool stay = (unsigned)(i - ha[r]) < (unsigned)(hb[r] - ha[r]);     // ha <= hb: the hint is non-decreasing
+            if (valid && !stay) mover_bits |= 1u << r;
+            if (valid && i < ha[r]) lo_bits |= 1u << r;
         }
     } else {
 #pragma unroll
         for (int r = 0; r < kClsIPT; ++r)
-            if (key[r] != 0xFFFFFFFFu) mover_bits |= 1u << r;
+            if (!CHECK || key[r] != 0xFFFFFFFFu) mover_bits |= 1u << r;
     }
 #pragma unroll
     for (int r = 0; r < kClsIPT; ++r) {
         // run-length aggregation of the histogram inside the warp
-        const bool valid = key[r] != 0xFFFFFFFFu;
         const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, key[r], 1);
         const bool head = (lane == 0) || (prev != key[r]);
         const unsigned heads = __ballot_sync(0xFFFFFFFFu, head);
-        if (head && valid) {
+        if (head && (!CHECK || key[r] != 0xFFFFFFFFu)) {
             const unsigned above = heads & ~((2u << lane) - 1);      // heads strictly above this lane
             const int next = above ? __ffs(above) - 1 : 32;
             // a run never extends over the invalid lanes of a ragged last word: those carry key
@@ -203,6 +178,28 @@ k_classify(PartP<T> p, GridP<T> g, int64_t n, const int32_t* __restrict__ old_of
         }
         bal[r] = __ballot_sync(0xFFFFFFFFu, (mover_bits >> r) & 1u);
     }
+}
+
+template <typename T, int D>
+__global__ void __launch_bounds__(kClsThreads)
+k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, int32_t* __restrict__ cell_count,
+           int32_t* __restrict__ mover_count, int32_t* __restrict__ mover_lo, uint32_t* __restrict__ mkey,
+           uint32_t* __restrict__ midx, uint32_t* __restrict__ mask, uint32_t* __restrict__ mprefix,
+           int32_t* __restrict__ tile_count, uint32_t* __restrict__ pkey, const uint32_t* __restrict__ counters)
+{
+    __shared__ uint32_t s_wsum[kClsWarps];
+    const unsigned tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tile = (int)blockIdx.x;
+    const bool hint_ok = counters[kCtrHintBad] == 0u;
+    const int wbase = tile * kClsTile + (int)warp * (32 * kClsIPT);
+
+    uint32_t key[kClsIPT], bal[kClsIPT];
+    uint32_t mover_bits, lo_bits;
+    if (wbase + 32 * kClsIPT <= n)
+        classify_warp<T, D, false>(p, g, n, wbase, lane, hint_ok, old_off, cell_count, pkey, key, bal, mover_bits, lo_bits);
+    else
+        classify_warp<T, D, true>(p, g, n, wbase, lane, hint_ok, old_off, cell_count, pkey, key, bal, mover_bits, lo_bits);
+
     // movers before each word of this warp, warp total
     uint32_t wpre[kClsIPT], wtotal = 0;
 #pragma unroll
@@ -219,19 +216,26 @@ k_classify(PartP<T> p, GridP<T> g, int64_t n, const int32_t* __restrict__ old_of
     if (tid == 0) tile_count[tile] = (int32_t)total;
     // tile-relative for now: k_movers_place adds the movers of the tiles before this one
     const uint32_t base = warp_off;
-    const int64_t stage = (int64_t)tile * kClsTile;
+    const int stage = tile * kClsTile;
     const unsigned lt = (1u << lane) - 1;
+    // lane r writes the mask and prefix words of row r (the ballots are the same in every lane)
+    {
+        uint32_t my_bal = 0, my_pre = 0;
+#pragma unroll
+        for (int r = 0; r < kClsIPT; ++r)
+            if ((int)lane == r) { my_bal = bal[r]; my_pre = wpre[r]; }
+        const int iw = wbase + (int)lane * 32;
+        if (lane < kClsIPT && iw < n) {
+            mask[iw >> 5] = my_bal;
+            mprefix[iw >> 5] = base + my_pre;
+        }
+    }
 #pragma unroll
     for (int r = 0; r < kClsIPT; ++r) {
-        const int64_t i0 = wbase + r * 32;
-        if (i0 < n && lane == 0) {
-            mask[i0 >> 5] = bal[r];
-            mprefix[i0 >> 5] = base + wpre[r];
-        }
         if ((mover_bits >> r) & 1u) {
-            const int64_t dst = stage + base + wpre[r] + __popc(bal[r] & lt);
+            const int dst = stage + (int)(base + wpre[r]) + __popc(bal[r] & lt);
             mkey[dst] = key[r];
-            midx[dst] = (uint32_t)(i0 + lane);
+            midx[dst] = (uint32_t)(wbase + r * 32 + (int)lane);
             atomicAdd(&mover_count[key[r]], 1);
             if ((lo_bits >> r) & 1u) atomicAdd(&mover_lo[key[r]], 1);
         }
@@ -522,78 +526,30 @@ __global__ void __launch_bounds__(256) k_perm_movers(const uint32_t* __restrict_
     }
 }
 
-// stayers: position i (mover bit clear) belongs to the cell k whose hint interval holds i, i.e.
-// k = (first cell of the tile) + #{cells whose interval ends at or before i}; that count is a
-// prefix sum over the tile of "interval ends here" marks
-__global__ void __launch_bounds__(kClsThreads)
-k_perm_stayers(const int32_t* __restrict__ old_off, const int32_t* __restrict__ tile_first, const int32_t* __restrict__ cell_base,
-               const uint32_t* __restrict__ mask, const uint32_t* __restrict__ mprefix, int32_t* __restrict__ perm, int C,
-               int64_t n, const uint32_t* __restrict__ counters)
+// stayers: position i (mover bit clear) kept its cell k = pkey[i] and goes to
+// cell_base[k] + i - (#movers before i).  Coalesced over positions; the mask word is one broadcast load.
+constexpr int kStayIPT = 4;
+__global__ void __launch_bounds__(256)
+k_perm_stayers(const uint32_t* __restrict__ pkey, const int32_t* __restrict__ cell_base, const uint32_t* __restrict__ mask,
+               const uint32_t* __restrict__ mprefix, int32_t* __restrict__ perm, int n, const uint32_t* __restrict__ counters)
 {
-    if (counters[kCtrHintBad]) return;
-    __shared__ int s_ends[kClsTile];                     // number of intervals ending at each position -> home cell
-    __shared__ int s_warp[kClsWarps];
-    __shared__ int s_more;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int64_t t0 = (int64_t)blockIdx.x * kClsTile;
-    const int64_t t1 = (t0 + kClsTile < n) ? t0 + kClsTile : n;
-    // anything to do?  (tiles made of movers only are common in the first, unsorted step)
-    bool any = false;
-    for (int64_t w = (t0 >> 5) + tid; w < ((t1 + 31) >> 5); w += kClsThreads) {
-        const int64_t left = t1 - (w << 5);
-        const uint32_t validbits = left >= 32 ? 0xFFFFFFFFu : ((1u << left) - 1u);
-        any = any || ((~mask[w]) & validbits) != 0u;
+    if (counters[kCtrHintBad]) return;                 // no stayers
+    const int base = ((int)blockIdx.x * 256 + (int)(threadIdx.x & ~31u)) * kStayIPT + (int)(threadIdx.x & 31u);
+    uint32_t m[kStayIPT], pre[kStayIPT], k[kStayIPT];
+#pragma unroll
+    for (int r = 0; r < kStayIPT; ++r) {
+        const int i = base + r * 32;
+        m[r] = i < n ? mask[i >> 5] : 0xFFFFFFFFu;
+        pre[r] = i < n ? mprefix[i >> 5] : 0u;
+        k[r] = i < n ? pkey[i] : 0u;
     }
-    if (!__syncthreads_or(any)) return;
-
-    for (int i = tid; i < kClsTile; i += kClsThreads) s_ends[i] = 0;
-    __syncthreads();
-    const int c0 = tile_first[blockIdx.x];
-    for (int kb = c0;; kb += kClsThreads) {              // cells c0, c0+1, ... until an interval ends beyond the tile
-        const int k = kb + tid;
-        bool more = false;
-        if (k < C) {
-            const int64_t b = old_off[k + 1];
-            if (b < t1) {
-                if (b >= t0) atomicAdd(&s_ends[(int)(b - t0)], 1);
-                more = true;                                // intervals are ordered: later cells may still end inside
-            }
-        }
-        if (tid == kClsThreads - 1) s_more = (more && k + 1 < C) ? 1 : 0;
-        __syncthreads();
-        const int go = s_more;
-        __syncthreads();
-        if (!go) break;
-    }
-    // inclusive prefix sum of s_ends over the tile (blocked: 8 consecutive positions per thread)
-    int v[kClsIPT], sum = 0;
+    const uint32_t bit = 1u << (threadIdx.x & 31u);
 #pragma unroll
-    for (int r = 0; r < kClsIPT; ++r) { sum += s_ends[tid * kClsIPT + r]; v[r] = sum; }
-    int inc = sum;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
-        if (lane >= o) inc += t;
-    }
-    if (lane == 31) s_warp[warp] = inc;
-    __syncthreads();
-    int off = c0 + inc - sum;
-    for (int w = 0; w < warp; ++w) off += s_warp[w];
-#pragma unroll
-    for (int r = 0; r < kClsIPT; ++r) s_ends[tid * kClsIPT + r] = off + v[r];
-    __syncthreads();
-    // coalesced over positions
-#pragma unroll
-    for (int r = 0; r < kClsIPT; ++r) {
-        const int loc = r * kClsThreads + tid;
-        const int64_t i = t0 + loc;
-        if (i < t1) {
-            const uint32_t m = mask[i >> 5];
-            if (!((m >> (i & 31)) & 1u)) {
-                const int k = s_ends[loc];
-                const uint32_t mv = mprefix[i >> 5] + __popc(m & ((1u << (i & 31)) - 1u));
-                perm[cell_base[k] + (int32_t)i - (int32_t)mv] = (int32_t)i;
-            }
+    for (int r = 0; r < kStayIPT; ++r) {
+        const int i = base + r * 32;
+        if (!(m[r] & bit)) {
+            const int mv = (int)(pre[r] + __popc(m[r] & (bit - 1u)));
+            perm[cell_base[k[r]] + i - mv] = i;
         }
     }
 }
@@ -633,7 +589,7 @@ static int64_t cells_of(const pic_grid_t& g)
 }
 
 struct SortLayout {
-    size_t keys0, keys1, idx0, idx1, mask, mprefix, old_off, mover_off, cell_base, tile_first, tile_count, tile_base, lookback;
+    size_t keys0, keys1, idx0, idx1, pkey, mask, mprefix, old_off, mover_off, cell_base, tile_count, tile_base, lookback;
     size_t zero_begin, cell_count, mover_count, mover_lo, digit_hist, scan_status, cls_status, counters, zero_end;
     size_t racc, total;
     int passes, bits, key_bits;
@@ -658,12 +614,12 @@ static SortLayout sort_layout(const pic_grid_t& g, int64_t n)
     L.keys1 = off; off += nb;
     L.idx0 = off; off += nb;
     L.idx1 = off; off += nb;
+    L.pkey = off; off += nb;
     L.mask = off; off += wb;
     L.mprefix = off; off += wb;
     L.old_off = off; off += cb;
     L.mover_off = off; off += cb;
     L.cell_base = off; off += cb;
-    L.tile_first = off; off += align256(sizeof(int32_t) * (size_t)(L.cls_tiles + 1));
     L.tile_count = off; off += align256(sizeof(int32_t) * (size_t)(L.cls_tiles + 1));
     L.tile_base = off; off += align256(sizeof(int32_t) * (size_t)(L.cls_tiles + 2));
     L.lookback = off; off += align256(sizeof(uint32_t) * (size_t)L.passes * (size_t)(L.radix_tiles > 0 ? L.radix_tiles : 1) * kRadix);
@@ -697,7 +653,7 @@ int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, Sor
     o.old_off = (int32_t*)(b + L.old_off);
     o.mover_off = (int32_t*)(b + L.mover_off);
     o.cell_base = (int32_t*)(b + L.cell_base);
-    o.tile_first = (int32_t*)(b + L.tile_first);
+    o.pkey = (uint32_t*)(b + L.pkey);
     o.tile_count = (int32_t*)(b + L.tile_count);
     o.tile_base = (int32_t*)(b + L.tile_base);
     o.lookback = (uint32_t*)(b + L.lookback);
@@ -732,16 +688,15 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
     k_hint_check<<<(unsigned)((C + 1 + 255) / 256), 256, 0, st>>>(cell_offsets, ws.old_off, C, n, ws.counters);
     count_launch();
     if (n > 0) {
-        k_hint_tiles<<<(unsigned)((C + 1 + 255) / 256), 256, 0, st>>>(ws.old_off, C, (int)ws.cls_tiles, ws.tile_first, ws.counters);
         // movers are staged per tile in the second halves of the ping-pong arrays, then packed
         k_classify<T, D><<<(unsigned)ws.cls_tiles, kClsThreads, 0, st>>>(
-            make_partp<T>(in), make_gridp<T>(g), n, ws.old_off, ws.cell_count, ws.mover_count, ws.mover_lo, ws.keys[1],
-            ws.idx[1], ws.mask, ws.mprefix, ws.tile_count, ws.counters);
+            make_partp<T>(in), make_gridp<T>(g), (int)n, ws.old_off, ws.cell_count, ws.mover_count, ws.mover_lo, ws.keys[1],
+            ws.idx[1], ws.mask, ws.mprefix, ws.tile_count, ws.pkey, ws.counters);
         k_scan_cells<<<(unsigned)((ws.cls_tiles + kScanTile - 1) / kScanTile), kScanThreads, 0, st>>>(
             ws.tile_count, ws.tile_base, (int)ws.cls_tiles, ws.cls_status, ws.counters + kCtrCls, nullptr, 0, 0);
         k_movers_place<<<(unsigned)ws.cls_tiles, kClsThreads, 0, st>>>(ws.keys[1], ws.idx[1], ws.keys[0], ws.idx[0], ws.mask,
                                                                       ws.mprefix, ws.tile_base, (int)ws.cls_tiles, n, ws.counters);
-        count_launch(4);
+        count_launch(3);
     }
     mark_phase(PIC_PHASE_KEYS, st);
     k_scan_cells<<<(unsigned)ws.scan_tiles, kScanThreads, 0, st>>>(ws.cell_count, cell_offsets, C, ws.scan_status,
@@ -772,8 +727,8 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
                                                                  ws.cell_base, C, ws.counters);
         k_perm_movers<<<148 * 8, 256, 0, st>>>(ws.keys[src], ws.idx[src], cell_offsets, ws.mover_off, ws.old_off, perm,
                                               ws.counters);
-        k_perm_stayers<<<(unsigned)ws.cls_tiles, kClsThreads, 0, st>>>(ws.old_off, ws.tile_first, ws.cell_base, ws.mask,
-                                                                      ws.mprefix, perm, C, n, ws.counters);
+        k_perm_stayers<<<(unsigned)((n + 256 * kStayIPT - 1) / (256 * kStayIPT)), 256, 0, st>>>(
+            ws.pkey, ws.cell_base, ws.mask, ws.mprefix, perm, (int)n, ws.counters);
         count_launch(3);
     }
     mark_phase(PIC_PHASE_REORDER, st);
