@@ -115,6 +115,7 @@ __global__ void __launch_bounds__(256) k_hint_check(const int32_t* __restrict__ 
 template <typename T, int D, bool CHECK>
 __device__ __forceinline__ void classify_warp(const PartP<T>& p, const GridP<T>& g, int n, int wbase, unsigned lane, bool hint_ok,
                                               const int32_t* __restrict__ old_off, int32_t* __restrict__ cell_count,
+                                              int32_t* __restrict__ mover_count, int32_t* __restrict__ mover_lo,
                                               uint32_t* __restrict__ pkey, uint32_t (&key)[kClsIPT], uint32_t (&bal)[kClsIPT],
                                               uint32_t& mover_bits, uint32_t& lo_bits)
 {
@@ -163,9 +164,34 @@ __device__ __forceinline__ void classify_warp(const PartP<T>& p, const GridP<T>&
         for (int r = 0; r < kClsIPT; ++r)
             if (!CHECK || key[r] != 0xFFFFFFFFu) mover_bits |= 1u << r;
     }
+    // the three histograms (all keys, movers, movers from below), aggregated inside the warp so that
+    // the number of atomics does not grow with the density (clustered config 4)
+    uint32_t lob[kClsIPT];
+    bool one_key = true;
 #pragma unroll
     for (int r = 0; r < kClsIPT; ++r) {
-        // run-length aggregation of the histogram inside the warp
+        bal[r] = __ballot_sync(0xFFFFFFFFu, (mover_bits >> r) & 1u);
+        lob[r] = __ballot_sync(0xFFFFFFFFu, (lo_bits >> r) & 1u);
+        one_key = one_key && key[r] == key[0];
+    }
+    const uint32_t k0 = __shfl_sync(0xFFFFFFFFu, key[0], 0);
+    one_key = __all_sync(0xFFFFFFFFu, one_key && key[0] == k0) && (!CHECK || k0 != 0xFFFFFFFFu);
+    if (one_key) {
+        // all 32*kClsIPT positions of the warp carry the same key: one atomic per histogram
+        if (lane == 0) {
+            int nm = 0, nl = 0;
+#pragma unroll
+            for (int r = 0; r < kClsIPT; ++r) { nm += __popc(bal[r]); nl += __popc(lob[r]); }
+            atomicAdd(&cell_count[k0], 32 * kClsIPT);
+            if (nm) atomicAdd(&mover_count[k0], nm);
+            if (nl) atomicAdd(&mover_lo[k0], nl);
+        }
+        return;
+    }
+#pragma unroll
+    for (int r = 0; r < kClsIPT; ++r) {
+        // one atomic per run of equal keys in a row of 32 positions (the common case once the
+        // particles are pre-ordered)
         const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, key[r], 1);
         const bool head = (lane == 0) || (prev != key[r]);
         const unsigned heads = __ballot_sync(0xFFFFFFFFu, head);
@@ -174,9 +200,12 @@ __device__ __forceinline__ void classify_warp(const PartP<T>& p, const GridP<T>&
             const int next = above ? __ffs(above) - 1 : 32;
             // a run never extends over the invalid lanes of a ragged last word: those carry key
             // 0xFFFFFFFF, so the first of them is a head
+            const unsigned run = (next == 32 ? 0xFFFFFFFFu : ((1u << next) - 1u)) & ~((1u << lane) - 1u);
             atomicAdd(&cell_count[key[r]], next - (int)lane);
+            const int nm = __popc(bal[r] & run), nl = __popc(lob[r] & run);
+            if (nm) atomicAdd(&mover_count[key[r]], nm);
+            if (nl) atomicAdd(&mover_lo[key[r]], nl);
         }
-        bal[r] = __ballot_sync(0xFFFFFFFFu, (mover_bits >> r) & 1u);
     }
 }
 
@@ -196,9 +225,11 @@ k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, i
     uint32_t key[kClsIPT], bal[kClsIPT];
     uint32_t mover_bits, lo_bits;
     if (wbase + 32 * kClsIPT <= n)
-        classify_warp<T, D, false>(p, g, n, wbase, lane, hint_ok, old_off, cell_count, pkey, key, bal, mover_bits, lo_bits);
+        classify_warp<T, D, false>(p, g, n, wbase, lane, hint_ok, old_off, cell_count, mover_count, mover_lo, pkey, key, bal,
+                                    mover_bits, lo_bits);
     else
-        classify_warp<T, D, true>(p, g, n, wbase, lane, hint_ok, old_off, cell_count, pkey, key, bal, mover_bits, lo_bits);
+        classify_warp<T, D, true>(p, g, n, wbase, lane, hint_ok, old_off, cell_count, mover_count, mover_lo, pkey, key, bal,
+                                    mover_bits, lo_bits);
 
     // movers before each word of this warp, warp total
     uint32_t wpre[kClsIPT], wtotal = 0;
@@ -236,8 +267,6 @@ k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, i
             const int dst = stage + (int)(base + wpre[r]) + __popc(bal[r] & lt);
             mkey[dst] = key[r];
             midx[dst] = (uint32_t)(wbase + r * 32 + (int)lane);
-            atomicAdd(&mover_count[key[r]], 1);
-            if ((lo_bits >> r) & 1u) atomicAdd(&mover_lo[key[r]], 1);
         }
     }
 }

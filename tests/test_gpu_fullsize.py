@@ -1,5 +1,5 @@
-"""Parity at BASELINE.json's full size, in the launch configuration bench.py times (cfg3: 3-D 128^3,
-1e8 particles, fp32, cubic, Stepper with ping-pong buffers, sort every step).
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (Stepper with
+ping-pong buffers, sort every step): cfg2, cfg3 (the headline), cfg4 (clustered) and cfg5 at 128 ppc.
 
 The oracle cannot run 1e8 particles in seconds, so this checks (i) what is unique and cheap to verify
 exactly at any size -- perm is a bijection, the keys of the reordered input are non-decreasing, perm is
@@ -29,12 +29,17 @@ def _keys_torch(x, n):
     return k
 
 
+def _full_cfg(name):
+    return W.cfg5(128, 1) if name == "cfg5" else W.CONFIGS[name]
+
+
 @pytest.mark.timeout(1200)
-def test_cfg3_full_size_two_steps():
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5"])
+def test_full_size_two_steps(name):
     import oracle as O
     import paper_1603_02886_b200 as B
 
-    cfg = W.CONFIGS["cfg3"]
+    cfg = _full_cfg(name)
     n, d = cfg.N, cfg.dim
     wl = W.make_workload(cfg)
     g, go = B.grid_of(cfg), O.grid_of(cfg)
@@ -67,7 +72,7 @@ def test_cfg3_full_size_two_steps():
         # (ii) charge conservation: sum rho h^d = sum w (fp32 rho rounded once per node)
         tot_w = float(before["w"].double().sum())
         tot_rho = float(st.rho.double().sum())
-        assert abs(tot_rho - tot_w) <= 1e-6 * tot_w
+        assert abs(tot_rho - tot_w) <= (1e-6 if cfg.dtype == "f32" else 1e-12) * tot_w
 
         # (iii-a) sampled particles: slot j of the output = pushed particle perm[j] of the input
         js = torch.from_numpy(rng.choice(n, 4096, replace=False)).cuda()
@@ -81,23 +86,32 @@ def test_cfg3_full_size_two_steps():
             assert err_v(st.cur["v"][c][js].cpu().numpy(), rv[c]) <= TOL_XV[cfg.dtype]
         assert torch.equal(st.cur["w"][js], before["w"][src])
 
-        # (iii-b) rho on the nodes of a sub-box, from the particles of the cells around it
-        lo, size, halo = (5 + 40 * step, 60, 125), 6, 3      # crosses nothing / the periodic seam in z
+        # (iii-b) rho on the nodes of a sub-box, from the particles of the cells around it (the box
+        #          crosses the periodic seam in the last dimension; cfg4: it sits inside the dense blob)
+        size, halo = 6, 3
+        nn = list(cfg.n) + [1] * (3 - d)
+        lo = [5 + 40 * step if nn[0] > 64 else 5 + 20 * step, nn[1] // 2 - 3, nn[2] - 3 if d == 3 else 0]
+        if d == 2:
+            lo[1] = nn[1] - 3
+        if cfg.clustered:                        # 1.5 sigma off the blob centre: a few thousand particles per cell
+            lo = [70, 70, 70 - 6 * step]
+        rng_z = range(lo[2] - halo, lo[2] + size + halo) if d == 3 else [0]
         cells = []
-        for kz in range(lo[2] - halo, lo[2] + size + halo):
+        for kz in rng_z:
             for ky in range(lo[1] - halo, lo[1] + size + halo):
-                base = (ky % cfg.n[1]) * cfg.n[0] + (kz % cfg.n[2]) * cfg.n[0] * cfg.n[1]
+                base = (ky % nn[1]) * nn[0] + (kz % nn[2]) * nn[0] * nn[1]
                 for kx in range(lo[0] - halo, lo[0] + size + halo):
-                    cells.append(base + kx % cfg.n[0])
+                    cells.append(base + kx % nn[0])
         cells = torch.tensor(sorted(set(cells)), device="cuda")
         a, b = off[cells], off[cells + 1]
         idx = torch.cat([perm[int(s):int(e)] for s, e in zip(a.tolist(), b.tolist())])
         xs = [before["x"][c][idx].cpu().numpy() for c in range(d)]
         ws = before["w"][idx].cpu().numpy()
-        rho_ref = O.deposit(go, xs, ws).reshape(cfg.n[2], cfg.n[1], cfg.n[0])
-        rho_gpu = st.rho.cpu().numpy().astype(np.float64).reshape(cfg.n[2], cfg.n[1], cfg.n[0])
-        zz = [(lo[2] + k) % cfg.n[2] for k in range(size)]
-        sub_ref = rho_ref[zz][:, lo[1]:lo[1] + size, lo[0]:lo[0] + size]
-        sub_gpu = rho_gpu[zz][:, lo[1]:lo[1] + size, lo[0]:lo[0] + size]
+        rho_ref = O.deposit(go, xs, ws).reshape(nn[2], nn[1], nn[0])
+        rho_gpu = st.rho.cpu().numpy().astype(np.float64).reshape(nn[2], nn[1], nn[0])
+        zz = [(lo[2] + k) % nn[2] for k in range(size if d == 3 else 1)]
+        yy = [(lo[1] + k) % nn[1] for k in range(size)]
+        sub_ref = rho_ref[zz][:, yy][:, :, lo[0]:lo[0] + size]
+        sub_gpu = rho_gpu[zz][:, yy][:, :, lo[0]:lo[0] + size]
         assert np.max(np.abs(sub_gpu - sub_ref)) <= TOL_RHO[cfg.dtype] * np.max(np.abs(rho_gpu))
         del before
