@@ -132,8 +132,13 @@ int pic_push(const pic_grid_t *grid, pic_particles_t *p, int order_state,
  * accel -> push, the paper's loop order setrho -> accel -> push with the
  * field solve left out as in the paper and the re-sort of PAPER.md:100 placed first (R6).
  * out receives the particles in sorted order, advanced to t+1; rho is the density at t.
- * do_sort = 0: particles keep their order (out_a[j] = advanced in_a[j]); perm is not written and
- * cell_offsets (which may be stale or NULL) is not modified.
+ * do_sort = 0: particles keep their order (out_a[j] = advanced in_a[j]; out may be the same arrays as
+ * in); perm is not written and cell_offsets is not modified.  cell_offsets may be NULL (any-order
+ * kernels) or the offsets of an EARLIER sort of these particles: they are then used to walk the
+ * particles cell by cell, and a particle that has left its cell since is taken on its own
+ * (threads-on-particles, setrho 3.3.4).  The result is exact whatever cell_offsets
+ * holds: offsets that cannot be walked (checked on the device: off[0] = 0, off[C] = N, non-decreasing)
+ * select the any-order kernels.  This is config 5's "sort every 4 / 16 steps" arm.
  */
 int pic_step(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t *out,
              int32_t *perm, int32_t *cell_offsets, void *rho, const void *const E[3],

@@ -207,6 +207,12 @@ int pic_step(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
         mark_phase(PIC_PHASE_PUSH, st);
         return rc;
     }
+    if (order_state == PIC_ORDER_STALE && in->n > 0) {
+        if (!aligned16(cell_offsets)) return PIC_ERR_INVALID_ARG;
+        rc = launch_stale_step(*grid, o, cell_offsets, rho, E, dt, qm, sws.racc, sws.gate, st);
+        mark_phase(PIC_PHASE_PUSH, st);
+        return rc;
+    }
     if ((rc = launch_deposit(*grid, o, order_state, cell_offsets, rho, sws.racc, st)) != PIC_OK) return rc;
     mark_phase(PIC_PHASE_DEPOSIT, st);
     rc = launch_push(*grid, o, order_state, cell_offsets, E, dt, qm, st);

@@ -501,10 +501,10 @@ inline int launch_group(const pic_grid_t& g, const pic_particles_t& src, const p
 template <typename T, int D, int P, int MODE, bool VIA_PERM>
 inline int launch_sorted(const pic_grid_t& g, const pic_particles_t& src, const pic_particles_t& dst,
                          const int32_t* perm, const int32_t* cell_offsets, const void* const E[3], double* racc,
-                         double dt, double qm, cudaStream_t st)
+                         double dt, double qm, cudaStream_t st, const uint32_t* gate = nullptr, uint32_t want = 0)
 {
 #if PIC_SORTED_KERNEL == 1
-    return launch_rows<T, D, P, MODE, VIA_PERM>(g, src, dst, perm, cell_offsets, E, racc, dt, qm, st);
+    return launch_rows<T, D, P, MODE, VIA_PERM>(g, src, dst, perm, cell_offsets, E, racc, dt, qm, st, gate, want);
 #else
     return launch_group<T, D, P, MODE, VIA_PERM>(g, src, dst, perm, cell_offsets, E, racc, dt, qm, st);
 #endif

@@ -1,11 +1,14 @@
-// pic_rows.cuh -- the sorted-order kernel, second design: LANES ON STENCIL ROWS.
+// pic_rows.cuh -- the kernel for particles grouped by cell: LANES ON STENCIL ROWS.
 //
-// Same job as k_tile (pic_tile.cuh): deposit and/or gather+accel+push over particles grouped by
-// cell (rows a5-a7, fused a8, optionally with the reorder a4 through perm).  k_tile keeps the S^d
-// node sums of a cell thread-private and pays for it with 64 accumulator registers,
-// a 56-shuffle combine per cell and 12 warps per SM.  Here the paper's other collision-free idea is
-// applied INSIDE a cell: "threads on splines" (setrho 3.3.1) -- every lane owns
-// grid nodes, not particles:
+// Deposit and/or gather+accel+push over particles sorted by cell (rows a5-a7, fused a8, optionally
+// with the reorder a4 through perm).  Prior art: the paper's CUDA kernel stages a per-block tile of
+// rho in shared memory and atomicAdds every particle's 8 products into it ("sorting is required",
+// PAPER.md:294, 504-525); it also names reducing "on a temporary thread-private variable"
+// (PAPER.md:300).  On sm_100a a floating-point atomicAdd on shared memory is a compare-and-swap
+// loop, and S^d thread-private sums per particle lane cost 64 registers and a combine per cell
+// (pic_group.cuh does that).  Here the paper's other collision-free idea is applied INSIDE a
+// cell: "threads on splines" (setrho 3.3.1) -- every lane owns grid nodes, not
+// particles:
 //
 //   * a warp owns WR consecutive slots of the sorted order, lists the cell runs inside them
 //     ("items", at most kItemMax particles, in cell order) and works through them NG = 32/G at a
@@ -26,7 +29,7 @@
 // Shared memory holds only the weight records and the item list (9 KB per warp), registers hold
 // RPL*S*(d+1) stencil values instead of S^d sums, so 16-20 warps fit on an SM.
 #pragma once
-#include "pic_tile.cuh"
+#include "pic_stencil.cuh"
 
 namespace pic {
 
@@ -127,9 +130,11 @@ constexpr int rows_min_blocks()
 template <typename T, int D, int P, int MODE, bool VIA_PERM, int G_>
 __global__ void __launch_bounds__(kRowsThreads, (rows_min_blocks<T, D, P, MODE, G_>()))
 k_rows(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g, FieldP<T> f,
-       const int32_t* __restrict__ cell_offsets, int64_t n, double* __restrict__ racc, T dt, T qmdt)
+       const int32_t* __restrict__ cell_offsets, int64_t n, double* __restrict__ racc, T dt, T qmdt,
+       const uint32_t* __restrict__ gate, uint32_t want)
 {
     using SH = RowsShape<T, D, P, G_>;
+    if (gate && *gate != want) return;                // the caller's cell_offsets failed the device-side check
     constexpr int S = SH::S, S2 = S / 2, SZ = SH::SZ;
     constexpr int G = SH::G, RPL = SH::RPL, NG = SH::NG, WR = SH::WR, REC = SH::REC;
     constexpr int kItemMax = SH::kItemMax;
@@ -420,11 +425,7 @@ k_rows(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
 
         // ---- end of the item: this lane's node sums go to the grid
         if constexpr (DEP) {
-#ifdef PIC_EXP_NORED
-            if (have && acc[0][0].r == 0x123456789abcdefull) {
-#else
             if (have) {
-#endif
 #pragma unroll
                 for (int rr = 0; rr < RPL; ++rr)
 #pragma unroll
@@ -443,7 +444,7 @@ k_rows(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
 template <typename T, int D, int P, int MODE, bool VIA_PERM>
 inline int launch_rows(const pic_grid_t& g, const pic_particles_t& src, const pic_particles_t& dst,
                        const int32_t* perm, const int32_t* cell_offsets, const void* const E[3], double* racc,
-                       double dt, double qm, cudaStream_t st)
+                       double dt, double qm, cudaStream_t st, const uint32_t* gate = nullptr, uint32_t want = 0)
 {
     if (dst.n <= 0) return PIC_OK;
     constexpr int GP = sizeof(T) == 4 ? PIC_ROWS_G32 : 8;
@@ -461,7 +462,7 @@ inline int launch_rows(const pic_grid_t& g, const pic_particles_t& src, const pi
     constexpr int64_t per_block = (int64_t)SH::WR * kRowsWarps;
     const unsigned blocks = (unsigned)((dst.n + per_block - 1) / per_block);
     kern<<<blocks, kRowsThreads, smem, st>>>(make_partp<T>(VIA_PERM ? src : dst), make_partp<T>(dst), perm,
-                                            make_gridp<T>(g), f, cell_offsets, dst.n, racc, (T)dt, (T)(qm * dt));
+                                            make_gridp<T>(g), f, cell_offsets, dst.n, racc, (T)dt, (T)(qm * dt), gate, want);
     count_launch();
     return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }

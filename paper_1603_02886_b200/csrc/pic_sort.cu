@@ -55,7 +55,7 @@ constexpr int kClsWarps = kClsThreads / 32;
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagPrefix = 2u << 30, kValMask = (1u << 30) - 1;
 
 // slots of SortWs::counters
-enum { kCtrScanA = 0, kCtrScanB = 1, kCtrCls = 2, kCtrRadix = 3 /* .. +kMaxPasses */, kCtrMovers = 8, kCtrHintBad = 9 };
+enum { kCtrScanA = 0, kCtrScanB = 1, kCtrCls = 2, kCtrRadix = 3 /* .. +kMaxPasses */, kCtrMovers = 8, kCtrHintBad = 9, kCtrGate = 16 };
 
 __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p)
 {
@@ -103,6 +103,27 @@ __global__ void __launch_bounds__(256) k_hint_check(const int32_t* __restrict__ 
     bool bad = a < 0 || (int64_t)a > n;
     if (k < C) bad = bad || hint[k + 1] < a;
     if (bad) counters[kCtrHintBad] = 1u;
+}
+
+// *gate = 1 unless off[0] = 0 <= off[1] <= ... <= off[C] = n (the caller zeroes *gate)
+__global__ void __launch_bounds__(256) k_offsets_check(const int32_t* __restrict__ off, int C, int64_t n, uint32_t* gate)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k > C) return;
+    const int32_t a = off[k];
+    bool bad = a < 0 || (int64_t)a > n || (k == 0 && a != 0) || (k == C && (int64_t)a != n);
+    if (k < C) bad = bad || off[k + 1] < a;
+    if (bad) *gate = 1u;
+}
+
+int launch_offsets_check(const pic_grid_t& g, const int32_t* cell_offsets, int64_t n, uint32_t* gate, cudaStream_t st)
+{
+    int64_t C = 1;
+    for (int c = 0; c < g.dim; ++c) C *= g.n[c];
+    PIC_CUDA_OK(cudaMemsetAsync(gate, 0, sizeof(uint32_t), st));
+    k_offsets_check<<<(unsigned)((C + 1 + 255) / 256), 256, 0, st>>>(cell_offsets, (int)C, n, gate);
+    count_launch();
+    return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
 
 // ----------------------------------------------------------------------------- keys, histograms, stayer/mover split
@@ -693,6 +714,7 @@ int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, Sor
     o.scan_status = (uint32_t*)(b + L.scan_status);
     o.cls_status = (uint32_t*)(b + L.cls_status);
     o.counters = (uint32_t*)(b + L.counters);
+    o.gate = o.counters + kCtrGate;
     o.zero_begin = b + L.zero_begin;
     o.zero_bytes = L.zero_end - L.zero_begin;
     o.racc = (double*)(b + L.racc);

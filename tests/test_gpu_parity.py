@@ -350,3 +350,39 @@ def test_argument_validation():
     ws = torch.empty(B.pic_workspace_bytes(g, n), dtype=torch.uint8, device="cuda")
     with pytest.raises(B.PicError):                                                   # in aliases out
         B.pic_sort(g, x, x, w, x, x, w, perm, off, ws)
+
+
+@pytest.mark.parametrize("kind", ["garbage", "not_covering", "stale"])
+def test_step_without_sort_any_cell_offsets(kind):
+    """pic_step(do_sort = 0) must be exact whatever cell_offsets holds: offsets that cannot be walked
+    (device-side check) fall back to the any-order kernels; offsets of an earlier sort are walked cell
+    by cell and the particles that left their cell since are taken one by one."""
+    O, B = _mods()
+    cfg = _cfg("cfg3", dict(N=150_000, n=(32, 32, 32)))
+    wl = W.make_workload(cfg)
+    go, gb = O.grid_of(cfg), B.grid_of(cfg)
+    n = cfg.N
+    x, v, w = wl.x, wl.v, wl.w
+    if kind == "stale":                       # sort, then advance twice without telling the offsets
+        r = O.step(go, x, v, w, wl.E, cfg.dt, cfg.qm)
+        off_host = r["cell_offsets"].copy()
+        x, v, w = r["x"], r["v"], r["w"]
+        r = O.step(go, x, v, w, wl.E, cfg.dt, cfg.qm, do_sort=False, cell_offsets=off_host)
+        x, v, w = r["x"], r["v"], r["w"]
+    elif kind == "garbage":
+        off_host = np.random.default_rng(3).integers(-5, n + 5, gb.cells + 1).astype(np.int32)
+    else:                                     # non-decreasing but off[C] != N: would skip particles
+        off_host = np.sort(np.random.default_rng(4).integers(0, n // 2, gb.cells + 1)).astype(np.int32)
+        off_host[0] = 0
+    ref = O.step(go, x, v, w, wl.E, cfg.dt, cfg.qm, do_sort=False, cell_offsets=off_host)
+    xi, vi, wi = to_dev(x), to_dev(v), to_dev([w])[0]
+    off = torch.from_numpy(np.concatenate([off_host, np.zeros(3, np.int32)])).cuda()
+    rho = torch.empty(gb.cells, dtype=gb.torch_dtype, device="cuda")
+    ws = torch.empty(B.pic_workspace_bytes(gb, n), dtype=torch.uint8, device="cuda")
+    B.pic_step(gb, xi, vi, wi, xi, vi, wi, None, off, rho, to_dev(wl.E), cfg.dt, cfg.qm, False, ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(off[: gb.cells + 1].cpu().numpy(), off_host)          # not modified
+    assert err_rho(rho.cpu().numpy(), ref["rho"]) <= TOL_RHO[cfg.dtype]
+    for c in range(cfg.dim):
+        assert err_x(xi[c].cpu().numpy(), ref["x"][c], cfg.L[c]) <= TOL_XV[cfg.dtype]
+        assert err_v(vi[c].cpu().numpy(), ref["v"][c]) <= TOL_XV[cfg.dtype]
