@@ -8,7 +8,7 @@
 // and counts 6 loads + 3 stores for each; fused they are
 // 2d loads + 2d stores per particle.  k_push_particles reads E through the read-only path
 // ("scattered reads through read-only data cache") and is correct for any order.
-#include "pic_group.cuh"
+#include "pic_rows.cuh"
 
 namespace pic {
 
@@ -66,7 +66,7 @@ static int push_impl(const pic_grid_t& g, pic_particles_t& p, int order_state, c
 {
     if (p.n > 0) {
         if (order_state == PIC_ORDER_SORTED)
-            return launch_sorted<T, D, P, kModePush, false>(g, p, p, nullptr, cell_offsets, E, nullptr, dt, qm, st);
+            return launch_rows<T, D, P, kModePush, false>(g, p, p, nullptr, cell_offsets, E, nullptr, dt, qm, st);
         FieldP<T> f;
         for (int c = 0; c < 3; ++c) f.E[c] = c < D ? (const T*)E[c] : nullptr;
         k_push_particles<T, D, P><<<(unsigned)((p.n + 255) / 256), 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), f, p.n,

@@ -6,7 +6,7 @@
 // PAPER.md:294, 504-525); it also names reducing "on a temporary thread-private variable"
 // (PAPER.md:300).  On sm_100a a floating-point atomicAdd on shared memory is a compare-and-swap
 // loop, and S^d thread-private sums per particle lane cost 64 registers and a combine per cell
-// (pic_group.cuh does that).  Here the paper's other collision-free idea is applied INSIDE a
+// (measured: slower).  Here the paper's other collision-free idea is applied INSIDE a
 // cell: "threads on splines" (setrho 3.3.1) -- every lane owns grid nodes, not
 // particles:
 //
@@ -276,7 +276,7 @@ k_rows(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
         T nx[D], nv[D], nw = (T)0;
 #pragma unroll
         for (int c = 0; c < D; ++c) { nx[c] = (T)0; nv[c] = (T)0; }
-        int in1 = 0, in2 = 0;                         // source index of this lane's particle in batch b+1, b+2
+        int in1 = 0;                                  // source index of this lane's particle in batch b+1 (then b+2)
         auto load_attrs = [&](int i) {
 #pragma unroll
             for (int c = 0; c < D; ++c) {
@@ -298,7 +298,8 @@ k_rows(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
             for (int c = 0; c < D; ++c) { px[c] = nx[c]; pv[c] = nv[c]; }
             // prefetch: attributes of batch b+1 (index known), index of batch b+2
             if (have && (b + 1) * G + lg < len) load_attrs(in1);
-            if (have && (b + 2) * G + lg < len) in2 = VIA_PERM ? perm[jbase + (b + 2) * G] : (int)jbase + (b + 2) * G;
+            // loaded straight into in1 (its old value has just been consumed): no copy of an in-flight load
+            if (have && (b + 2) * G + lg < len) in1 = VIA_PERM ? perm[jbase + (b + 2) * G] : (int)jbase + (b + 2) * G;
 
             // ---- phase W: lane = particle
             bool same = true;
@@ -420,7 +421,6 @@ k_rows(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
                     if constexpr (VIA_PERM) dst.w[j] = pw;
                 }
             }
-            in1 = in2;
         }
 
         // ---- end of the item: this lane's node sums go to the grid

@@ -1,5 +1,5 @@
 // pic_stencil.cuh -- pieces shared by the kernels that work on particles grouped by cell
-// (pic_rows.cuh, pic_group.cuh) and by the any-order kernels: field pointers, kernel modes, the
+// (pic_rows.cuh) and by the any-order kernels: field pointers, kernel modes, the
 // stencil width of a cell, packed pairs, the 1-D spline weights of a cell's stencil.
 //
 // S = stencil width of a CELL: 2 for p = 1, 4 for p = 2, 3 (a quadratic particle touches 3 of the
@@ -47,12 +47,14 @@ __device__ __forceinline__ float pk_lo(Pk<float> p)
 {
     float lo, hi;
     asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(p.r));
+    (void)hi;
     return lo;
 }
 __device__ __forceinline__ float pk_hi(Pk<float> p)
 {
     float lo, hi;
     asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(p.r));
+    (void)lo;
     return hi;
 }
 __device__ __forceinline__ double pk_lo(Pk<double> p) { return p.lo; }
