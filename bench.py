@@ -61,8 +61,8 @@ def measured_peaks():
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r01_v3_rows.md): key = "<config>:<phase of the dominant kernel>"
-NCU_TRAFFIC = {"cfg3:push": 8.32e9}
+# `ncu --set full` capture (profiles/r01_v4_final.md): key = "<config>:<phase of the dominant kernel>"
+NCU_TRAFFIC = {"cfg3:push": 8.32e9}          # 5.13 GB read + 3.19 GB written (profiles/r01_v4_final.md)
 
 
 def ncu_traffic(cfg_name, kernel):
@@ -176,7 +176,7 @@ def replica_throughput(n_per_rank, world, steps, ms_total_max):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg3")
@@ -186,7 +186,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-particles", type=int, default=2_000_000)
-    ap.add_argument("--cpu-particles", type=int, default=10_000_000)
+    ap.add_argument("--cpu-particles", type=int, default=30_000_000)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
