@@ -132,11 +132,39 @@ int launch_offsets_check(const pic_grid_t& g, const int32_t* cell_offsets, int64
 // case once the particles are pre-ordered) are merged into one atomic per run.
 // Movers (see the header) are appended to (mkey, midx) in position order; mask / mprefix hold,
 // per 32 positions, the movers' bits and the number of movers before the word.
+// Per-block hash table key -> (count, movers, movers from below) in shared memory (open addressing, 8 probes;
+// a key that finds no slot goes straight to the global histograms).  Counts of a block are at most
+// kClsTile = 2^12: count and movers share one word (13 bits each).
+constexpr int kHashBits = 10, kHashSize = 1 << kHashBits;
+struct BlockHist {
+    uint32_t* key;      // [kHashSize], 0xFFFFFFFF = empty
+    uint32_t* c01;      // [kHashSize] count | movers << 13
+    uint32_t* c2;       // [kHashSize] movers from below
+    int32_t *cell_count, *mover_count, *mover_lo;
+    __device__ __forceinline__ void add(uint32_t k, uint32_t c0, uint32_t c1, uint32_t cl) const
+    {
+        uint32_t slot = (k * 2654435761u) >> (32 - kHashBits);
+#pragma unroll 1
+        for (int probe = 0; probe < 8; ++probe) {
+            const uint32_t old = atomicCAS(&key[slot], 0xFFFFFFFFu, k);
+            if (old == 0xFFFFFFFFu || old == k) {
+                atomicAdd(&c01[slot], c0 | (c1 << 13));
+                if (cl) atomicAdd(&c2[slot], cl);
+                return;
+            }
+            slot = (slot + 1) & (kHashSize - 1);
+        }
+        atomicAdd(&cell_count[k], (int)c0);
+        if (c1) atomicAdd(&mover_count[k], (int)c1);
+        if (cl) atomicAdd(&mover_lo[k], (int)cl);
+    }
+};
+static_assert(kClsTile <= (1 << 12), "13-bit fields of BlockHist");
+
 // One warp's 32*kClsIPT positions.  CHECK = false: all of them are below n (no bounds tests).
 template <typename T, int D, bool CHECK>
 __device__ __forceinline__ void classify_warp(const PartP<T>& p, const GridP<T>& g, int n, int wbase, unsigned lane, bool hint_ok,
-                                              const int32_t* __restrict__ old_off, int32_t* __restrict__ cell_count,
-                                              int32_t* __restrict__ mover_count, int32_t* __restrict__ mover_lo,
+                                              const int32_t* __restrict__ old_off, const BlockHist& hist,
                                               uint32_t* __restrict__ pkey, uint32_t (&key)[kClsIPT], uint32_t (&bal)[kClsIPT],
                                               uint32_t& mover_bits, uint32_t& lo_bits)
 {
@@ -185,34 +213,19 @@ __device__ __forceinline__ void classify_warp(const PartP<T>& p, const GridP<T>&
         for (int r = 0; r < kClsIPT; ++r)
             if (!CHECK || key[r] != 0xFFFFFFFFu) mover_bits |= 1u << r;
     }
-    // the three histograms (all keys, movers, movers from below), aggregated inside the warp so that
-    // the number of atomics does not grow with the density (clustered config 4)
-    uint32_t lob[kClsIPT];
-    bool one_key = true;
+    // the three histograms (all keys, movers, movers from below): one entry per run of equal keys in a
+    // row of 32 positions (the common case once the particles are pre-ordered) goes to the
+    // block's hash table in shared memory; the table is flushed with one global atomic per key and
+    // histogram, so the number of global atomics on one address does not grow with the density (clustered
+    // config 4: same-address atomics serialise in L2 and made this kernel 3.7x slower)
+    // (dense = the warp's 512 positions span at most three cells; elsewhere the addresses are spread and the
+    // atomics go straight to the grid arrays, which is cheaper than hashing)
+    const uint32_t kfirst = __shfl_sync(0xFFFFFFFFu, key[0], 0), klast = __shfl_sync(0xFFFFFFFFu, key[kClsIPT - 1], 31);
+    const bool dense = klast - kfirst <= 2u;
 #pragma unroll
     for (int r = 0; r < kClsIPT; ++r) {
         bal[r] = __ballot_sync(0xFFFFFFFFu, (mover_bits >> r) & 1u);
-        lob[r] = __ballot_sync(0xFFFFFFFFu, (lo_bits >> r) & 1u);
-        one_key = one_key && key[r] == key[0];
-    }
-    const uint32_t k0 = __shfl_sync(0xFFFFFFFFu, key[0], 0);
-    one_key = __all_sync(0xFFFFFFFFu, one_key && key[0] == k0) && (!CHECK || k0 != 0xFFFFFFFFu);
-    if (one_key) {
-        // all 32*kClsIPT positions of the warp carry the same key: one atomic per histogram
-        if (lane == 0) {
-            int nm = 0, nl = 0;
-#pragma unroll
-            for (int r = 0; r < kClsIPT; ++r) { nm += __popc(bal[r]); nl += __popc(lob[r]); }
-            atomicAdd(&cell_count[k0], 32 * kClsIPT);
-            if (nm) atomicAdd(&mover_count[k0], nm);
-            if (nl) atomicAdd(&mover_lo[k0], nl);
-        }
-        return;
-    }
-#pragma unroll
-    for (int r = 0; r < kClsIPT; ++r) {
-        // one atomic per run of equal keys in a row of 32 positions (the common case once the
-        // particles are pre-ordered)
+        const unsigned lob = __ballot_sync(0xFFFFFFFFu, (lo_bits >> r) & 1u);
         const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, key[r], 1);
         const bool head = (lane == 0) || (prev != key[r]);
         const unsigned heads = __ballot_sync(0xFFFFFFFFu, head);
@@ -222,16 +235,20 @@ __device__ __forceinline__ void classify_warp(const PartP<T>& p, const GridP<T>&
             // a run never extends over the invalid lanes of a ragged last word: those carry key
             // 0xFFFFFFFF, so the first of them is a head
             const unsigned run = (next == 32 ? 0xFFFFFFFFu : ((1u << next) - 1u)) & ~((1u << lane) - 1u);
-            atomicAdd(&cell_count[key[r]], next - (int)lane);
-            const int nm = __popc(bal[r] & run), nl = __popc(lob[r] & run);
-            if (nm) atomicAdd(&mover_count[key[r]], nm);
-            if (nl) atomicAdd(&mover_lo[key[r]], nl);
+            const uint32_t c0 = (uint32_t)(next - (int)lane), c1 = (uint32_t)__popc(bal[r] & run), cl = (uint32_t)__popc(lob & run);
+            if (dense) {
+                hist.add(key[r], c0, c1, cl);
+            } else {
+                atomicAdd(&hist.cell_count[key[r]], (int)c0);
+                if (c1) atomicAdd(&hist.mover_count[key[r]], (int)c1);
+                if (cl) atomicAdd(&hist.mover_lo[key[r]], (int)cl);
+            }
         }
     }
 }
 
 template <typename T, int D>
-__global__ void __launch_bounds__(kClsThreads)
+__global__ void __launch_bounds__(kClsThreads, 3)
 k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, int32_t* __restrict__ cell_count,
            int32_t* __restrict__ mover_count, int32_t* __restrict__ mover_lo, uint32_t* __restrict__ mkey,
            uint32_t* __restrict__ midx, uint32_t* __restrict__ mask, uint32_t* __restrict__ mprefix,
@@ -243,14 +260,17 @@ k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, i
     const bool hint_ok = counters[kCtrHintBad] == 0u;
     const int wbase = tile * kClsTile + (int)warp * (32 * kClsIPT);
 
+    __shared__ uint32_t s_hkey[kHashSize], s_hc01[kHashSize], s_hc2[kHashSize];
+    for (int q = tid; q < kHashSize; q += kClsThreads) { s_hkey[q] = 0xFFFFFFFFu; s_hc01[q] = 0u; s_hc2[q] = 0u; }
+    __syncthreads();
+    const BlockHist hist{s_hkey, s_hc01, s_hc2, cell_count, mover_count, mover_lo};
+
     uint32_t key[kClsIPT], bal[kClsIPT];
     uint32_t mover_bits, lo_bits;
     if (wbase + 32 * kClsIPT <= n)
-        classify_warp<T, D, false>(p, g, n, wbase, lane, hint_ok, old_off, cell_count, mover_count, mover_lo, pkey, key, bal,
-                                    mover_bits, lo_bits);
+        classify_warp<T, D, false>(p, g, n, wbase, lane, hint_ok, old_off, hist, pkey, key, bal, mover_bits, lo_bits);
     else
-        classify_warp<T, D, true>(p, g, n, wbase, lane, hint_ok, old_off, cell_count, mover_count, mover_lo, pkey, key, bal,
-                                    mover_bits, lo_bits);
+        classify_warp<T, D, true>(p, g, n, wbase, lane, hint_ok, old_off, hist, pkey, key, bal, mover_bits, lo_bits);
 
     // movers before each word of this warp, warp total
     uint32_t wpre[kClsIPT], wtotal = 0;
@@ -266,6 +286,16 @@ k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, i
         total += t;
     }
     if (tid == 0) tile_count[tile] = (int32_t)total;
+    // the block's histograms go to the grid arrays: one atomic per key and histogram (after the barrier above)
+    for (int q = tid; q < kHashSize; q += kClsThreads) {
+        const uint32_t k = s_hkey[q];
+        if (k != 0xFFFFFFFFu) {
+            const uint32_t v = s_hc01[q], l = s_hc2[q];
+            atomicAdd(&cell_count[k], (int)(v & 0x1FFFu));
+            if (v >> 13) atomicAdd(&mover_count[k], (int)(v >> 13));
+            if (l) atomicAdd(&mover_lo[k], (int)l);
+        }
+    }
     // tile-relative for now: k_movers_place adds the movers of the tiles before this one
     const uint32_t base = warp_off;
     const int stage = tile * kClsTile;
