@@ -115,3 +115,56 @@ def test_full_size_two_steps(name):
         sub_gpu = rho_gpu[zz][:, yy][:, :, lo[0]:lo[0] + size]
         assert np.max(np.abs(sub_gpu - sub_ref)) <= TOL_RHO[cfg.dtype] * np.max(np.abs(rho_gpu))
         del before
+
+
+@pytest.mark.timeout(1800)
+@pytest.mark.parametrize("ppc", [8, 32, 128, 512])
+@pytest.mark.parametrize("k", [1, 4, 16])
+def test_cfg5_sweep_17_steps(ppc, k):
+    """Config 5 at full size: ppc in {8, 32, 128, 512} x sort every k in {1, 4, 16} steps, 17 steps (one
+    re-sort at k = 16 is crossed).  Every step: exact charge conservation of rho; on sort steps the sort
+    post-conditions; on the last two steps (one of them a step without sort for k > 1) sampled particles
+    against the oracle's push."""
+    import oracle as O
+    import paper_1603_02886_b200 as B
+
+    cfg = W.cfg5(ppc, k)
+    n, d = cfg.N, cfg.dim
+    wl = W.make_workload(cfg)
+    g, go = B.grid_of(cfg), O.grid_of(cfg)
+    st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, device="cuda:0")
+    tot_w = float(st.cur["w"].double().sum())
+    rng = np.random.default_rng(11)
+    for step in range(17):
+        do_sort = step % k == 0
+        check = step >= 15
+        if check:
+            js = torch.from_numpy(rng.choice(n, 2048, replace=False)).cuda()
+            if do_sort:
+                x_in = [a.clone() for a in st.cur["x"]]
+                v_in = [a.clone() for a in st.cur["v"]]
+            else:
+                x_in = [a[js].clone() for a in st.cur["x"]]
+                v_in = [a[js].clone() for a in st.cur["v"]]
+        st.step(cfg.dt, cfg.qm, do_sort)
+        torch.cuda.synchronize()
+        assert abs(float(st.rho.double().sum()) - tot_w) <= 1e-12 * tot_w, "charge not conserved at step %d" % step
+        if do_sort and (step == 0 or check):
+            perm = st.perm[:n].to(torch.int64)
+            seen = torch.zeros(n, dtype=torch.uint8, device="cuda")
+            seen[perm] = 1
+            assert int(seen.sum()) == n
+            off = st.cell_offsets[: g.cells + 1].to(torch.int64)
+            assert int(off[0]) == 0 and int(off[-1]) == n and bool((off[1:] >= off[:-1]).all())
+        if check:
+            if do_sort:
+                src = st.perm[:n].to(torch.int64)[js]
+                xs = [a[src].cpu().numpy() for a in x_in]
+                vs = [a[src].cpu().numpy() for a in v_in]
+            else:
+                xs = [a.cpu().numpy() for a in x_in]
+                vs = [a.cpu().numpy() for a in v_in]
+            rx, rv = O.push(go, xs, vs, wl.E, cfg.dt, cfg.qm)
+            for c in range(d):
+                assert err_x(st.cur["x"][c][js].cpu().numpy(), rx[c], cfg.L[c]) <= TOL_XV[cfg.dtype]
+                assert err_v(st.cur["v"][c][js].cpu().numpy(), rv[c]) <= TOL_XV[cfg.dtype]
