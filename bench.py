@@ -311,6 +311,12 @@ def main():
             dist.destroy_process_group()
         return
 
+    # config 5 asks for the deposit with and without sorting (the paper's sorted vs unsorted columns,
+    # PAPER.md:392-394): pic_deposit on the current sorted order, and on the never-sorted initial order
+    deposit_compare = None
+    if args.config == "cfg5" and world == 1:
+        deposit_compare = run_deposit_compare(B, torch, cfg, g, wl, st, dev)
+
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
         cpu_baseline = run_cpu_baseline(cfg, args.cpu_particles)
@@ -323,6 +329,8 @@ def main():
             "step_roofline": {"bytes_per_particle_step": bytes_step, "achieved": step_ach, "peak": peak,
                               "frac": step_ach / peak, "frac_of_8TBps_nominal": step_ach / 8000.0, "unit": "GB/s"},
             "phase_ms": phase_ms, "first_step_ms": first_ms}
+    if deposit_compare:
+        line["deposit_ms"] = deposit_compare
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -361,6 +369,33 @@ def run_e2e(B, torch, cfg, g, wl, dev, K, world, dist):
     return {"value": n * world * steps / el, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
             "steps": steps, "ms_per_step": 1e3 * el / steps,
             "api": "pic_step_host (pinned host buffers, sort every step)"}
+
+
+def run_deposit_compare(B, torch, cfg, g, wl, st, dev, reps=5):
+    """ms per pic_deposit call: particles sorted by cell (per-cell kernel) against the same workload never
+    sorted (threads on particles with global atomics, setrho 3.3.4)."""
+    def timed(f):
+        f()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            f()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    a = st.cur
+    xs = [torch.empty_like(t) for t in a["x"]]
+    vs = [torch.empty_like(t) for t in a["v"]]
+    ws_ = torch.empty_like(a["w"])
+    B.pic_sort(g, a["x"], a["v"], a["w"], xs, vs, ws_, st.perm, st.cell_offsets, st.ws)
+    t_sorted = timed(lambda: B.pic_deposit(g, xs, ws_, st.rho, B.PIC_ORDER_SORTED, st.cell_offsets, st.ws))
+    del vs
+    x0 = [torch.from_numpy(np.ascontiguousarray(t)).to(dev) for t in wl.x]
+    w0 = torch.from_numpy(np.ascontiguousarray(wl.w)).to(dev)
+    t_unsorted = timed(lambda: B.pic_deposit(g, x0, w0, st.rho, B.PIC_ORDER_UNSORTED, None, st.ws))
+    return {"sorted": t_sorted, "never_sorted": t_unsorted, "unit": "ms per deposit of all particles"}
 
 
 def run_cpu_baseline(cfg, sample):
