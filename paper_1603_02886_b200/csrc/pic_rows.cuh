@@ -36,13 +36,16 @@ namespace pic {
 #ifndef PIC_ROWS_G32
 #define PIC_ROWS_G32 4          // lanes per item, fp32
 #endif
-#ifndef PIC_ROWS_MINB32
-#define PIC_ROWS_MINB32 3       // resident blocks per SM the fp32 kernels are compiled for
+#ifndef PIC_ROWS_MINW32
+#define PIC_ROWS_MINW32 12      // resident warps per SM the fp32 kernels are compiled for (168 registers)
 #endif
 #ifndef PIC_ROWS_WR
 #define PIC_ROWS_WR 1024
 #endif
-constexpr int kRowsWarps = 4;
+#ifndef PIC_ROWS_WARPS
+#define PIC_ROWS_WARPS 1        // warps per block (warps are independent; one-warp blocks measured best)
+#endif
+constexpr int kRowsWarps = PIC_ROWS_WARPS;
 constexpr int kRowsThreads = 32 * kRowsWarps;
 
 template <typename T, int D, int P, int G_>
@@ -124,7 +127,7 @@ __device__ __noinline__ void stray_from_regs(T x0, T x1, T x2, T v0, T v1, T v2,
 template <typename T, int D, int P, int MODE, int G_>
 constexpr int rows_min_blocks()
 {
-    return sizeof(T) == 4 ? PIC_ROWS_MINB32 : 2;
+    return (sizeof(T) == 4 ? PIC_ROWS_MINW32 : 8) / PIC_ROWS_WARPS;
 }
 
 template <typename T, int D, int P, int MODE, bool VIA_PERM, int G_>
