@@ -39,7 +39,10 @@ static inline size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 
 // ----------------------------------------------------------------------------- tile shapes
 constexpr int kRadixThreads = 256;
-constexpr int kRadixIPT = 16;
+#ifndef PIC_RADIX_IPT
+#define PIC_RADIX_IPT 16
+#endif
+constexpr int kRadixIPT = PIC_RADIX_IPT;
 constexpr int kRadixTile = kRadixThreads * kRadixIPT;      // 4096 pairs per tile
 constexpr int kRadixWarps = kRadixThreads / 32;
 
@@ -48,7 +51,10 @@ constexpr int kScanIPT = 8;
 constexpr int kScanTile = kScanThreads * kScanIPT;         // 2048 counts per tile
 
 constexpr int kClsThreads = 256;
-constexpr int kClsIPT = 16;
+#ifndef PIC_CLS_IPT
+#define PIC_CLS_IPT 16
+#endif
+constexpr int kClsIPT = PIC_CLS_IPT;
 constexpr int kClsTile = kClsThreads * kClsIPT;            // 4096 positions per tile
 constexpr int kClsWarps = kClsThreads / 32;
 
