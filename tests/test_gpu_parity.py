@@ -386,3 +386,78 @@ def test_step_without_sort_any_cell_offsets(kind):
     for c in range(cfg.dim):
         assert err_x(xi[c].cpu().numpy(), ref["x"][c], cfg.L[c]) <= TOL_XV[cfg.dtype]
         assert err_v(vi[c].cpu().numpy(), ref["v"][c]) <= TOL_XV[cfg.dtype]
+
+
+@pytest.mark.parametrize("h", [0.5, 0.3, 3.0])
+@pytest.mark.parametrize("name,kw", [("cfg2", dict(N=60_000, n=(48, 40))), ("cfg3", dict(N=90_000, n=(24, 20, 12)))])
+def test_step_lockstep_grid_spacing(name, kw, h):
+    """Spacing h != 1 (reading R13): a power of two takes the multiply path, 0.3 and 3.0 the IEEE division
+    in the storage precision; grids whose sizes are not powers of two; three steps in lockstep."""
+    _lockstep(_cfg(name, dict(kw, h=h)), 3)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("case", ["one_cell", "minimal_grid", "fast", "edges"])
+def test_step_degenerate(case, dtype):
+    """The degenerate cases of the method: every particle in one cell (one long run cut into pieces), the
+    smallest legal grid (n = p + 1: the stencil covers the whole grid), velocities that cross many boxes per
+    step, particles exactly on 0 and on the last representable position below L."""
+    O, B = _mods()
+    rng = np.random.default_rng(5)
+    dt_np = np.float64 if dtype == "f64" else np.float32
+    order = 3
+    n = (4, 4, 4) if case == "minimal_grid" else (12, 10, 8)
+    N = 20_000
+    cfg = W.CONFIGS["cfg3"].scaled(N, n=n, dtype=dtype, order=order)
+    L = np.array(n, np.float64)
+    x = [(rng.random(N) * L[c]).astype(dt_np) for c in range(3)]
+    v = [rng.normal(0, 1, N).astype(dt_np) for c in range(3)]
+    if case == "one_cell":
+        x = [(3.0 + rng.random(N)).astype(dt_np) for c in range(3)]
+    if case == "fast":
+        # several boxes per step.  In fp32 the push is computed in fp32 (the paper's precision switch, PAPER.md:479-482):
+        # its error is an ulp of |x + dt v|, so the 1e-6 L tolerance holds while |x + dt v| stays within a few L
+        v = [rng.normal(0, 400 if dtype == "f64" else 30, N).astype(dt_np) for c in range(3)]
+    if case == "edges":
+        for c in range(3):
+            x[c][0::4] = 0
+            x[c][1::4] = np.nextafter(dt_np(L[c]), dt_np(0))
+    for c in range(3):
+        x[c][x[c] >= L[c]] = 0
+    w = (0.5 + rng.random(N)).astype(dt_np)
+    E = [rng.normal(0, 1, cfg.cells).astype(dt_np) for c in range(3)]
+    go, gb = O.grid_of(cfg), B.grid_of(cfg)
+    ref = O.step(go, x, v, w, E, cfg.dt, cfg.qm)
+    xi, vi, wi = to_dev(x), to_dev(v), to_dev([w])[0]
+    xo, vo, wo = [torch.empty_like(a) for a in xi], [torch.empty_like(a) for a in vi], torch.empty_like(wi)
+    perm = torch.full((N,), -1, dtype=torch.int32, device="cuda")
+    off = torch.full((gb.cells + 4,), -1, dtype=torch.int32, device="cuda")
+    rho = torch.empty(gb.cells, dtype=gb.torch_dtype, device="cuda")
+    ws = torch.empty(B.pic_workspace_bytes(gb, N), dtype=torch.uint8, device="cuda")
+    for rep in range(2):          # second call: cell_offsets now holds a valid hint for the same input
+        B.pic_step(gb, xi, vi, wi, xo, vo, wo, perm, off, rho, to_dev(E), cfg.dt, cfg.qm, True, ws)
+        torch.cuda.synchronize()
+        assert np.array_equal(perm.cpu().numpy(), ref["perm"])
+        assert np.array_equal(off[: gb.cells + 1].cpu().numpy(), ref["cell_offsets"])
+        assert err_rho(rho.cpu().numpy(), ref["rho"]) <= TOL_RHO[dtype]
+        for c in range(3):
+            assert err_x(xo[c].cpu().numpy(), ref["x"][c], L[c]) <= TOL_XV[dtype]
+            assert err_v(vo[c].cpu().numpy(), ref["v"][c], sigma_v=max(1.0, float(np.max(np.abs(ref["v"][c]))))) <= TOL_XV[dtype]
+            xs = xo[c].cpu().numpy()
+            assert xs.min() >= 0 and xs.max() < L[c]
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_step_random_shapes(seed):
+    """Seeded random combinations of dimension, spline order, dtype, grid sizes (down to n = p + 1, odd sizes),
+    spacing, particle count (ragged tails), clustered or uniform: two steps in lockstep against the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    dim = int(rng.integers(2, 4))
+    order = int(rng.integers(1, 4))
+    dtype = "f64" if rng.random() < 0.5 else "f32"
+    n = tuple(int(rng.integers(order + 1, 40 if dim == 2 else 14)) for _ in range(dim))
+    N = int(rng.integers(1, 60_000))
+    h = float(rng.choice([1.0, 0.25, 0.7]))
+    base = "cfg2" if dim == 2 else ("cfg4" if rng.random() < 0.3 and min(n) >= 8 else "cfg3")
+    cfg = W.CONFIGS[base].scaled(N, n=n, order=order, dtype=dtype, h=h, seed=seed)
+    _lockstep(cfg, 2)
