@@ -306,6 +306,11 @@ def main():
     if not args.no_e2e:
         e2e = run_e2e(B, torch, cfg_rank, g, wl, dev, K, world, dist if world > 1 else None)
 
+    # ---- the same with the particles resident on the device: per step E goes in, rho comes out
+    e2e_resident = None
+    if not args.no_e2e:
+        e2e_resident = run_e2e_resident(B, torch, cfg_rank, g, wl, st, dev, K, world, dist if world > 1 else None)
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -331,6 +336,8 @@ def main():
             "phase_ms": phase_ms, "first_step_ms": first_ms}
     if deposit_compare:
         line["deposit_ms"] = deposit_compare
+    if e2e_resident:
+        line["e2e_resident_particles"] = e2e_resident
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -369,6 +376,35 @@ def run_e2e(B, torch, cfg, g, wl, dev, K, world, dist):
     return {"value": n * world * steps / el, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
             "steps": steps, "ms_per_step": 1e3 * el / steps,
             "api": "pic_step_host (pinned host buffers, sort every step)"}
+
+
+def run_e2e_resident(B, torch, cfg, g, wl, st, dev, K, world, dist):
+    """Same metric through pic_step_fields_host: the particles stay on the device (the paper's arrangement,
+    PAPER.md:65, 447); every step copies the field E from pinned host memory to the device, runs the step and
+    reads rho back.  Wall clock around K synchronous calls."""
+    n = cfg.N
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    E = [pin(a) for a in wl.E]
+    rho = torch.empty(g.cells, dtype=g.torch_dtype).pin_memory()
+    ws = torch.empty(B.pic_step_fields_host_bytes(g, n), dtype=torch.uint8, device=dev)
+    a, b = st.cur, st.nxt
+    steps = max(1, K)
+    for k in range(2 + steps):
+        if k == 2:
+            if dist is not None:
+                dist.barrier()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+        B.pic_step_fields_host(g, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], st.perm, st.cell_offsets, rho, E,
+                               cfg.dt, cfg.qm, True, ws)
+        a, b = b, a
+    torch.cuda.synchronize()
+    el = max_over_ranks(time.perf_counter() - t0, dist, dev)
+    st.cur, st.nxt = a, b
+    s = g.itemsize
+    return {"value": n * world * steps / el, "unit": UNIT, "h2d_bytes_per_step": cfg.dim * s * g.cells,
+            "d2h_bytes_per_step": s * g.cells, "steps": steps, "ms_per_step": 1e3 * el / steps,
+            "api": "pic_step_fields_host (particles resident on the device; E in, rho out, pinned host buffers)"}
 
 
 def run_deposit_compare(B, torch, cfg, g, wl, st, dev, reps=5):

@@ -156,6 +156,20 @@ int pic_step_host(const pic_grid_t *grid, const pic_particles_t *in, pic_particl
                   double dt, double qm, int do_sort, void *dev_ws, size_t dev_ws_bytes,
                   void *stream);
 
+/*
+ * pic_step_fields_host -- one step with the particles RESIDENT on the device and the grid quantities
+ * on the host, the paper's arrangement: particle and grid arrays stay on the GPU ("present", PAPER.md:447;
+ * transfers "kept to a minimum") while the field comes from a solver outside.
+ * Copies E (HOST, each [C]) to the device, runs pic_step on the DEVICE arrays in / out / perm /
+ * cell_offsets exactly as pic_step does, copies rho (HOST, [C]) back and synchronises the stream.
+ * ws: DEVICE, at least pic_step_fields_host_bytes() bytes (the grids + the pic_step workspace).
+ */
+int pic_step_fields_host_bytes(const pic_grid_t *grid, int64_t n, size_t *bytes /* host, out */);
+int pic_step_fields_host(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t *out,
+                         int32_t *perm, int32_t *cell_offsets, void *rho /* host */,
+                         const void *const E[3] /* host */, double dt, double qm, int do_sort,
+                         void *ws, size_t ws_bytes, void *stream);
+
 /* Number of kernels the last call of this thread enqueued (for bench.py's gpu_launches). */
 int pic_last_launch_count(void);
 

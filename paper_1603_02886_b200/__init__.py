@@ -20,7 +20,8 @@ PIC_OK = 0
 PIC_ORDER_UNSORTED, PIC_ORDER_SORTED, PIC_ORDER_STALE = 0, 1, 2
 
 EXPORTS = ("pic_workspace_bytes", "pic_sort", "pic_deposit", "pic_push", "pic_step",
-           "pic_step_host_bytes", "pic_step_host", "pic_last_launch_count", "pic_set_phase_events",
+           "pic_step_host_bytes", "pic_step_host", "pic_step_fields_host_bytes", "pic_step_fields_host",
+           "pic_last_launch_count", "pic_set_phase_events",
            "pic_strerror")
 PHASES = ("begin", "keys", "scan", "radix", "reorder", "deposit", "push")
 
@@ -71,6 +72,8 @@ def lib():
         L.pic_step.argtypes = [G, P, P, vp, vp, vp, E3, dbl, dbl, ci, vp, sz, vp]
         L.pic_step_host_bytes.argtypes = [G, i64, ctypes.POINTER(sz)]
         L.pic_step_host.argtypes = [G, P, P, vp, vp, vp, E3, dbl, dbl, ci, vp, sz, vp]
+        L.pic_step_fields_host_bytes.argtypes = [G, i64, ctypes.POINTER(sz)]
+        L.pic_step_fields_host.argtypes = [G, P, P, vp, vp, vp, E3, dbl, dbl, ci, vp, sz, vp]
         L.pic_last_launch_count.argtypes = []
         L.pic_set_phase_events.argtypes = [ctypes.POINTER(ctypes.c_void_p), ci]
         L.pic_strerror.argtypes = [ci]
@@ -256,6 +259,26 @@ def pic_step_host(g: Grid, x_in, v_in, w_in, x_out, v_out, w_out, perm, cell_off
     _check(lib().pic_step_host(ctypes.byref(cg), ctypes.byref(pi), ctypes.byref(po), _ptr(perm), _ptr(cell_offsets),
                                _ptr(rho), _field(g, E), dt, qm, 1 if do_sort else 0, _ptr(dev_ws),
                                dev_ws.numel() * dev_ws.element_size(), _stream(stream)), "pic_step_host")
+
+
+def pic_step_fields_host_bytes(g: Grid, n: int) -> int:
+    out = ctypes.c_size_t(0)
+    cg = g.c()
+    _check(lib().pic_step_fields_host_bytes(ctypes.byref(cg), n, ctypes.byref(out)), "pic_step_fields_host_bytes")
+    return out.value
+
+
+def pic_step_fields_host(g: Grid, x_in, v_in, w_in, x_out, v_out, w_out, perm, cell_offsets, rho_host, E_host,
+                         dt: float, qm: float, do_sort: bool, ws, stream=None):
+    """pic_step with the particles on the device (CUDA tensors) and E, rho on the host (numpy / pinned tensors)."""
+    n = w_in.numel()
+    _dev_check(g, list(x_in) + list(v_in) + [w_in] + list(x_out) + list(v_out) + [w_out], n)
+    cg = g.c()
+    pi, po = _particles(g, x_in, v_in, w_in, n), _particles(g, x_out, v_out, w_out, n)
+    _check(lib().pic_step_fields_host(ctypes.byref(cg), ctypes.byref(pi), ctypes.byref(po), _ptr(perm),
+                                      _ptr(cell_offsets), _ptr(rho_host), _field(g, E_host), dt, qm,
+                                      1 if do_sort else 0, _ptr(ws), ws.numel() * ws.element_size(), _stream(stream)),
+           "pic_step_fields_host")
 
 
 class Stepper:

@@ -319,4 +319,44 @@ int pic_step_host(const pic_grid_t* grid, const pic_particles_t* in, pic_particl
     return PIC_OK;
 }
 
+// ---- particles resident on the device, grid quantities on the host --------------------------
+int pic_step_fields_host_bytes(const pic_grid_t* grid, int64_t n, size_t* bytes)
+{
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if (!bytes || n < 0 || n >= ((int64_t)1 << 30)) return PIC_ERR_INVALID_ARG;
+    const size_t s = grid->dtype == PIC_F64 ? 8 : 4;
+    *bytes = 4 * align256(s * (size_t)cells_of(*grid)) + sort_ws_bytes(*grid, n);
+    return PIC_OK;
+}
+
+int pic_step_fields_host(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t* out, int32_t* perm,
+                         int32_t* cell_offsets, void* rho, const void* const E[3], double dt, double qm, int do_sort,
+                         void* ws, size_t ws_bytes, void* stream)
+{
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if (!rho || !E || !aligned16(ws)) return PIC_ERR_INVALID_ARG;
+    const size_t s = grid->dtype == PIC_F64 ? 8 : 4;
+    const size_t C = (size_t)cells_of(*grid), gb = align256(s * C);
+    const size_t need = 4 * gb + sort_ws_bytes(*grid, in ? in->n : 0);
+    if (!in || ws_bytes < need) return in ? PIC_ERR_WORKSPACE : PIC_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    char* b = (char*)ws;
+    const void* dE[3] = {nullptr, nullptr, nullptr};
+    for (int c = 0; c < grid->dim; ++c) {
+        if (!E[c]) return PIC_ERR_INVALID_ARG;
+        dE[c] = b + (size_t)c * gb;
+        PIC_CUDA_OK(cudaMemcpyAsync(b + (size_t)c * gb, E[c], s * C, cudaMemcpyHostToDevice, st));
+    }
+    void* drho = b + 3 * gb;
+    rc = pic_step(grid, in, out, perm, cell_offsets, drho, dE, dt, qm, do_sort, b + 4 * gb, ws_bytes - 4 * gb, stream);
+    if (rc != PIC_OK) return rc;
+    const int launches = g_launches;
+    PIC_CUDA_OK(cudaMemcpyAsync(rho, drho, s * C, cudaMemcpyDeviceToHost, st));
+    PIC_CUDA_OK(cudaStreamSynchronize(st));
+    g_launches = launches;
+    return PIC_OK;
+}
+
 }  // extern "C"

@@ -461,3 +461,35 @@ def test_step_random_shapes(seed):
     base = "cfg2" if dim == 2 else ("cfg4" if rng.random() < 0.3 and min(n) >= 8 else "cfg3")
     cfg = W.CONFIGS[base].scaled(N, n=n, order=order, dtype=dtype, h=h, seed=seed)
     _lockstep(cfg, 2)
+
+
+def test_step_fields_host_entry_point():
+    """pic_step_fields_host: particles on the device, E and rho on the host; two steps (ping-pong) against the oracle."""
+    O, B = _mods()
+    cfg = _cfg("cfg3", dict(N=70_001, n=(16, 16, 16)))
+    wl = W.make_workload(cfg)
+    go, gb = O.grid_of(cfg), B.grid_of(cfg)
+    n = cfg.N
+    a = dict(x=to_dev(wl.x), v=to_dev(wl.v), w=to_dev([wl.w])[0])
+    b = dict(x=[torch.empty_like(t) for t in a["x"]], v=[torch.empty_like(t) for t in a["v"]], w=torch.empty_like(a["w"]))
+    perm = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    off = torch.full((gb.cells + 4,), -1, dtype=torch.int32, device="cuda")
+    ws = torch.empty(B.pic_step_fields_host_bytes(gb, n), dtype=torch.uint8, device="cuda")
+    rho = np.empty(gb.cells, cfg.np_dtype)
+    x, v, w = wl.x, wl.v, wl.w
+    for step in range(2):
+        ref = O.step(go, x, v, w, wl.E, cfg.dt, cfg.qm)
+        B.pic_step_fields_host(gb, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], perm, off, rho, wl.E,
+                               cfg.dt, cfg.qm, True, ws)
+        assert B.pic_last_launch_count() > 0
+        assert np.array_equal(perm.cpu().numpy(), ref["perm"])
+        assert err_rho(rho, ref["rho"]) <= TOL_RHO[cfg.dtype]
+        for c in range(cfg.dim):
+            assert err_x(b["x"][c].cpu().numpy(), ref["x"][c], cfg.L[c]) <= TOL_XV[cfg.dtype]
+            assert err_v(b["v"][c].cpu().numpy(), ref["v"][c]) <= TOL_XV[cfg.dtype]
+        # lockstep: the next step starts from the oracle's state
+        x, v, w = ref["x"], ref["v"], ref["w"]
+        a = dict(x=to_dev(x), v=to_dev(v), w=to_dev([w])[0])
+    with pytest.raises(B.PicError, match="workspace"):
+        B.pic_step_fields_host(gb, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], perm, off, rho, wl.E,
+                               cfg.dt, cfg.qm, True, ws[: 4096])
