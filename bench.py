@@ -298,6 +298,19 @@ def main():
                     "frac": ach / peak, "traffic": ncu_traffic(cfg.name, dom),
                     "peak_source": peak_src, "algorithmic_bytes_per_particle": bpp,
                     "kernel_ms": phase_ms[dom]}
+    # second roof of the dominant kernel: plain fp32/fp64 arithmetic.  Algorithmic flops
+    # per particle of deposit + gather on the (p+1)^d stencil: products 1, deposit FMA 2, gather FMAs 2d.
+    roofline_alu = None
+    if dom == "push" and B.FUSED_PHASE_IS_PUSH:
+        nodes = (cfg.order + 1) ** cfg.dim
+        flop_pp = nodes * (1 + 2 + 2 * cfg.dim)
+        sm_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
+        lanes = 128 if cfg.dtype == "f32" else 64
+        peak_tf = 148 * lanes * 2 * sm_mhz * 1e6 / 1e12
+        ach_tf = flop_pp * cfg.N / (phase_ms[dom] * 1e-3) / 1e12
+        roofline_alu = {"bound": "alu", "kernel": dom, "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                        "frac": ach_tf / peak_tf, "flop_per_particle": flop_pp,
+                        "peak_source": "148 SMs x %d lanes x 2 flop x SM clock (DESIGN.md section 6)" % lanes}
     bytes_step = ab["step"] if cfg.sort_every == 1 else (ab["step"] * sorts + ab["nosort_step"] * (K - sorts)) / K
     step_ach = bytes_step * cfg.N / (ms_step * 1e-3) / 1e9
 
@@ -338,6 +351,8 @@ def main():
         line["deposit_ms"] = deposit_compare
     if e2e_resident:
         line["e2e_resident_particles"] = e2e_resident
+    if roofline_alu:
+        line["roofline_alu"] = roofline_alu
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
