@@ -462,7 +462,10 @@ __global__ void __launch_bounds__(256) k_zero_lookback(uint32_t* lookback, const
 // (warp, round, lane) = ascending input position, so equal digits keep their input order.
 // keys_out == nullptr: keys are not needed any more (last pass).  The number of pairs is read
 // from the device (counters[kCtrMovers]); blocks beyond the last tile exit at once.
-__global__ void __launch_bounds__(kRadixThreads)
+#ifndef PIC_RADIX_MINB
+#define PIC_RADIX_MINB 5        // resident blocks per SM k_radix_pass is compiled for (48 registers)
+#endif
+__global__ void __launch_bounds__(kRadixThreads, PIC_RADIX_MINB)
 k_radix_pass(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ idx_in,
              uint32_t* __restrict__ keys_out, uint32_t* __restrict__ idx_out, const uint32_t* __restrict__ counters,
              int shift, uint32_t mask, const uint32_t* __restrict__ digit_offsets, uint32_t* tile_counter,
@@ -614,7 +617,10 @@ __global__ void __launch_bounds__(256) k_perm_movers(const uint32_t* __restrict_
 
 // stayers: position i (mover bit clear) kept its cell k = pkey[i] and goes to
 // cell_base[k] + i - (#movers before i).  Coalesced over positions; the mask word is one broadcast load.
-constexpr int kStayIPT = 4;
+#ifndef PIC_STAY_IPT
+#define PIC_STAY_IPT 4
+#endif
+constexpr int kStayIPT = PIC_STAY_IPT;
 __global__ void __launch_bounds__(256)
 k_perm_stayers(const uint32_t* __restrict__ pkey, const int32_t* __restrict__ cell_base, const uint32_t* __restrict__ mask,
                const uint32_t* __restrict__ mprefix, int32_t* __restrict__ perm, int n, const uint32_t* __restrict__ counters)
