@@ -254,7 +254,10 @@ __device__ __forceinline__ void classify_warp(const PartP<T>& p, const GridP<T>&
 }
 
 template <typename T, int D>
-__global__ void __launch_bounds__(kClsThreads, 3)
+#ifndef PIC_CLS_MINB
+#define PIC_CLS_MINB 4
+#endif
+__global__ void __launch_bounds__(kClsThreads, PIC_CLS_MINB)
 k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, int32_t* __restrict__ cell_count,
            int32_t* __restrict__ mover_count, int32_t* __restrict__ mover_lo, uint32_t* __restrict__ mkey,
            uint32_t* __restrict__ midx, uint32_t* __restrict__ mask, uint32_t* __restrict__ mprefix,
