@@ -61,8 +61,8 @@ def measured_peaks():
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r01_v4_final.md): key = "<config>:<phase of the dominant kernel>"
-NCU_TRAFFIC = {"cfg3:push": 8.32e9}          # 5.13 GB read + 3.19 GB written (profiles/r01_v4_final.md)
+# `ncu --set full` capture (profiles/r01_v5_final.md): key = "<config>:<phase of the dominant kernel>"
+NCU_TRAFFIC = {"cfg3:push": 8.38e9}          # 5.18 GB read + 3.20 GB written (profiles/r01_v5_final.md)
 
 
 def ncu_traffic(cfg_name, kernel):
