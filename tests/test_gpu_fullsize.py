@@ -168,3 +168,52 @@ def test_cfg5_sweep_17_steps(ppc, k):
             for c in range(d):
                 assert err_x(st.cur["x"][c][js].cpu().numpy(), rx[c], cfg.L[c]) <= TOL_XV[cfg.dtype]
                 assert err_v(st.cur["v"][c][js].cpu().numpy(), rv[c]) <= TOL_XV[cfg.dtype]
+
+
+@pytest.mark.timeout(1800)
+def test_maximum_particle_count():
+    """N = 2^30 - 1, the largest count the C ABI accepts (32-bit indices): fp32, 3-D 256^3, linear splines, inputs
+    drawn on the device (test-only: no oracle value is involved).  Two steps -- all particles movers, then the
+    incremental sort -- checked by what is exact at any size: perm is a bijection, cell_offsets is the scan of the
+    key histogram, keys of the reordered input are sorted, charge is conserved."""
+    import paper_1603_02886_b200 as B
+
+    free, _ = torch.cuda.mem_get_info()
+    if free < 150e9:
+        pytest.skip("needs about 130 GB of device memory")
+    n = (1 << 30) - 1
+    g = B.Grid(3, (256, 256, 256), (1.0, 1.0, 1.0), 1, "f32")
+    gen = torch.Generator(device="cuda").manual_seed(1)
+    mk = lambda scale: torch.rand(n, device="cuda", generator=gen, dtype=torch.float32) * scale
+    a = dict(x=[mk(256.0).clamp_(max=255.99998) for _ in range(3)],
+             v=[torch.randn(n, device="cuda", generator=gen, dtype=torch.float32) for _ in range(3)], w=mk(1.0) + 0.5)
+    b = dict(x=[torch.empty_like(t) for t in a["x"]], v=[torch.empty_like(t) for t in a["v"]], w=torch.empty_like(a["w"]))
+    E = [torch.randn(g.cells, device="cuda", generator=gen, dtype=torch.float32) * 0.1 for _ in range(3)]
+    perm = torch.empty(n, dtype=torch.int32, device="cuda")
+    off = torch.zeros(g.cells + 4, dtype=torch.int32, device="cuda")
+    rho = torch.empty(g.cells, dtype=torch.float32, device="cuda")
+    ws = torch.empty(B.pic_workspace_bytes(g, n), dtype=torch.uint8, device="cuda")
+    for step in range(2):
+        keys = None
+        for c, m in zip(range(3), (1, 256, 65536)):
+            kc = torch.floor(a["x"][c]).to(torch.int32).clamp_(0, 255) * m
+            keys = kc if keys is None else keys.add_(kc)
+            del kc
+        tot_w = float(a["w"].sum(dtype=torch.float64))
+        B.pic_step(g, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], perm, off, rho, E, 0.1, 1.0, True, ws)
+        torch.cuda.synchronize()
+        cnt = torch.bincount(keys, minlength=g.cells)
+        assert torch.equal(off[1: g.cells + 1].to(torch.int64), torch.cumsum(cnt, 0)) and int(off[0]) == 0
+        del cnt
+        seen = torch.zeros(n, dtype=torch.uint8, device="cuda")
+        seen[perm.to(torch.int64)] = 1
+        assert int(seen.sum(dtype=torch.int64)) == n, "perm is not a bijection"
+        del seen
+        skey = keys[perm.to(torch.int64)]
+        del keys
+        assert bool((skey[1:] >= skey[:-1]).all())
+        del skey
+        assert abs(float(rho.sum(dtype=torch.float64)) - tot_w) <= 2e-6 * tot_w
+        for c in range(3):
+            assert float(b["x"][c].min()) >= 0.0 and float(b["x"][c].max()) < 256.0
+        a, b = b, a
