@@ -69,6 +69,16 @@ __device__ __forceinline__ Pk<double> pk_fma(Pk<double> a, Pk<double> b, Pk<doub
 {
     return Pk<double>{fma(a.lo, b.lo, c.lo), fma(a.hi, b.hi, c.hi)};
 }
+// c += a * b in place (the accumulator is one read-write operand: no copy of a loop-carried sum)
+__device__ __forceinline__ void pk_acc(Pk<float>& c, Pk<float> a, Pk<float> b)
+{
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c.r) : "l"(a.r), "l"(b.r));
+}
+__device__ __forceinline__ void pk_acc(Pk<double>& c, Pk<double> a, Pk<double> b)
+{
+    c.lo = fma(a.lo, b.lo, c.lo);
+    c.hi = fma(a.hi, b.hi, c.hi);
+}
 __device__ __forceinline__ Pk<float> pk_mul(Pk<float> a, Pk<float> b)
 {
     Pk<float> d;
@@ -129,6 +139,78 @@ __device__ __forceinline__ void load_row(const T* __restrict__ p, Pk<T> (&e)[S /
             e[i] = pk_make(v.x, v.y);
         }
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// shared memory by 32-bit shared-window address.  The base is taken once with a volatile asm, so it
+// stays in a register (the compiler otherwise re-derives it from SR_CgaCtaId at every use).
+__device__ __forceinline__ uint32_t smem_base(const void* p)
+{
+    uint32_t a;
+    asm volatile("{ .reg .u64 t; cvta.to.shared.u64 t, %1; cvt.u32.u64 %0, t; }" : "=r"(a) : "l"(p));
+    return a;
+}
+// N consecutive elements of T at byte address a (aligned to min(16, N*sizeof(T)))
+template <typename T, int N>
+__device__ __forceinline__ void lds(uint32_t a, T (&o)[N])
+{
+    if constexpr (sizeof(T) == 4 && N % 4 == 0) {
+#pragma unroll
+        for (int i = 0; i < N / 4; ++i)
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                         : "=f"(o[4 * i]), "=f"(o[4 * i + 1]), "=f"(o[4 * i + 2]), "=f"(o[4 * i + 3]) : "r"(a + 16 * i));
+    } else if constexpr (sizeof(T) == 4 && N % 2 == 0) {
+#pragma unroll
+        for (int i = 0; i < N / 2; ++i)
+            asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(o[2 * i]), "=f"(o[2 * i + 1]) : "r"(a + 8 * i));
+    } else if constexpr (sizeof(T) == 4) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(o[i]) : "r"(a + 4 * i));
+    } else if constexpr (N % 2 == 0) {
+#pragma unroll
+        for (int i = 0; i < N / 2; ++i)
+            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(o[2 * i]), "=d"(o[2 * i + 1]) : "r"(a + 16 * i));
+    } else {
+#pragma unroll
+        for (int i = 0; i < N; ++i) asm volatile("ld.shared.f64 %0, [%1];" : "=d"(o[i]) : "r"(a + 8 * i));
+    }
+}
+template <typename T>
+__device__ __forceinline__ T lds1(uint32_t a)
+{
+    T v[1];
+    lds<T, 1>(a, v);
+    return v[0];
+}
+template <typename T, int N>
+__device__ __forceinline__ void sts(uint32_t a, const T (&o)[N])
+{
+    if constexpr (sizeof(T) == 4 && N % 4 == 0) {
+#pragma unroll
+        for (int i = 0; i < N / 4; ++i)
+            asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};"
+                         :: "r"(a + 16 * i), "f"(o[4 * i]), "f"(o[4 * i + 1]), "f"(o[4 * i + 2]), "f"(o[4 * i + 3]) : "memory");
+    } else if constexpr (sizeof(T) == 4 && N % 2 == 0) {
+#pragma unroll
+        for (int i = 0; i < N / 2; ++i)
+            asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(a + 8 * i), "f"(o[2 * i]), "f"(o[2 * i + 1]) : "memory");
+    } else if constexpr (sizeof(T) == 4) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) asm volatile("st.shared.f32 [%0], %1;" :: "r"(a + 4 * i), "f"(o[i]) : "memory");
+    } else if constexpr (N % 2 == 0) {
+#pragma unroll
+        for (int i = 0; i < N / 2; ++i)
+            asm volatile("st.shared.v2.f64 [%0], {%1, %2};" :: "r"(a + 16 * i), "d"(o[2 * i]), "d"(o[2 * i + 1]) : "memory");
+    } else {
+#pragma unroll
+        for (int i = 0; i < N; ++i) asm volatile("st.shared.f64 [%0], %1;" :: "r"(a + 8 * i), "d"(o[i]) : "memory");
+    }
+}
+template <typename T>
+__device__ __forceinline__ void sts1(uint32_t a, T v)
+{
+    const T o[1] = {v};
+    sts<T, 1>(a, o);
 }
 
 // rho[k] = (T) racc[k]

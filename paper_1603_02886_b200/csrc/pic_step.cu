@@ -3,7 +3,10 @@
 // particle perm[j] of src is read, slot j of p is written).  Legal because E is prescribed and frozen ("particles move
 // into a frozen given electric field"): rho(x^t) and the push of x^t
 // read the same particle data once.  Kernel: k_rows<MODE = deposit|push> (pic_rows.cuh).
+#include <cstdlib>
+
 #include "pic_rows.cuh"
+#include "pic_runs.cuh"
 
 namespace pic {
 
@@ -17,8 +20,14 @@ static int fused_impl(const pic_grid_t& g, const pic_particles_t& src, pic_parti
     double* racc = sizeof(T) == 8 ? (double*)rho : racc_ws;
     if (!racc) return PIC_ERR_WORKSPACE;
     PIC_CUDA_OK(cudaMemsetAsync(racc, 0, sizeof(double) * (size_t)C, st));
-    int rc = perm ? launch_rows<T, D, P, kModeBoth, true>(g, src, p, perm, cell_offsets, E, racc, dt, qm, st)
+    static const bool old_kernel = getenv("PIC_OLD_ROWS") != nullptr;      // TEMP: A/B switch
+    int rc;
+    if (old_kernel)
+        rc = perm ? launch_rows<T, D, P, kModeBoth, true>(g, src, p, perm, cell_offsets, E, racc, dt, qm, st)
                   : launch_rows<T, D, P, kModeBoth, false>(g, p, p, nullptr, cell_offsets, E, racc, dt, qm, st);
+    else
+        rc = perm ? launch_runs<T, D, P, kModeBoth, true>(g, src, p, perm, E, racc, dt, qm, st)
+                  : launch_runs<T, D, P, kModeBoth, false>(g, p, p, nullptr, E, racc, dt, qm, st);
     if (rc != PIC_OK) return rc;
     if (sizeof(T) == 4) {
         k_round_rho<T><<<(unsigned)((C + 255) / 256), 256, 0, st>>>(racc, (T*)rho, C);
