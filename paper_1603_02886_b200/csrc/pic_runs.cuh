@@ -179,7 +179,6 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
     // a new cell anywhere: every column is flushed and fetched
     auto jump_to = [&](int nx_, int ny_, int nz_) {
         int nnew[NPL];
-        T ev[NPL][PUSH ? D : 1];
         const int rho = (nx_ - sh) & (S - 1);
 #pragma unroll
         for (int m = 0; m < NPL; ++m) {
@@ -190,10 +189,6 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
             const int gy = fold(ny_ - sh + jy, g.n[1]);
             const int gz = (D == 3) ? fold(nz_ - sh + kz, g.n[2]) : 0;
             nnew[m] = gx + g.n[0] * (gy + g.n[1] * gz);
-            if constexpr (PUSH) {
-#pragma unroll
-                for (int c = 0; c < D; ++c) ev[m][c] = __ldg(f.E[c] + nnew[m]);    // in flight during the flush
-            }
         }
         if (DEP && since > 0) flush_all();
 #pragma unroll
@@ -206,12 +201,18 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
         }
         ccx = nx_; ccy = ny_; ccz = nz_;
         if constexpr (PUSH) {
+            cp_async_wait();                          // (a column fetched ahead for the old row is dropped)
+            if (lane < ROWS) {                        // the column the next slide will need
+                const int xnext = fold(ccx - sh + S, g.n[0]);
+#pragma unroll
+                for (int c = 0; c < D; ++c) cp_async_elem(a_col + (uint32_t)(c * ROWS + lane) * B, f.E[c] + rowb + xnext);
+            }
 #pragma unroll
             for (int m = 0; m < NPL; ++m) {
                 const int nid = lane + 32 * m;
                 if (NODES % 32 == 0 || nid < NODES) {
 #pragma unroll
-                    for (int c = 0; c < D; ++c) sts1<T>(a_buf + (uint32_t)(c * NODES + nid) * B, ev[m][c]);
+                    for (int c = 0; c < D; ++c) sts1<T>(a_buf + (uint32_t)(c * NODES + nid) * B, ldg_here(f.E[c] + nidx[m]));
                 }
             }
             __syncwarp();
@@ -232,13 +233,6 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
         const int rho = (ccx - sh) & (S - 1);
         const int xold = fold(ccx - sh, g.n[0]), xnew = fold(ccx - sh + S, g.n[0]);
         const bool rown = lane < ROWS;
-        T ev[PUSH ? D : 1];
-        if constexpr (PUSH) {
-            if (rown) {
-#pragma unroll
-                for (int c = 0; c < D; ++c) ev[c] = __ldg(f.E[c] + rowb + xnew);
-            }
-        }
         if (DEP && since > 0) {
             T col[RPL];
 #pragma unroll
@@ -257,10 +251,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
             }
         }
         if constexpr (PUSH) {
-            if (rown) {
-#pragma unroll
-                for (int c = 0; c < D; ++c) sts1<T>(a_col + (uint32_t)(c * ROWS + lane) * B, ev[c]);
-            }
+            cp_async_wait();                          // the column was fetched ahead, see below and jump_to
         }
         __syncwarp();
         if constexpr (PUSH) {
@@ -282,7 +273,14 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
             for (int m = 0; m < NPL; ++m) nidx[m] += xnew - xold;
         }
         ccx += 1;
-        if constexpr (PUSH) __syncwarp();             // the column buffer may be written again at once
+        if constexpr (PUSH) {
+            __syncwarp();                             // every lane has read the column: fetch the next one ahead
+            if (rown) {
+                const int xnext = fold(ccx - sh + S, g.n[0]);
+#pragma unroll
+                for (int c = 0; c < D; ++c) cp_async_elem(a_col + (uint32_t)(c * ROWS + lane) * B, f.E[c] + rowb + xnext);
+            }
+        }
     };
 
     // particle of this lane in the current batch, and the prefetched one of the next batch
@@ -432,6 +430,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
         }
     }
     if (DEP && since > 0) flush_all();
+    if constexpr (PUSH) cp_async_wait();              // a column fetched ahead may still be in flight
 }
 
 // launch k_runs over n particles.  VIA_PERM: particle perm[j] of src -> slot j of dst; otherwise in place

@@ -43,6 +43,14 @@ __device__ __forceinline__ Pk<float> pk_make(float lo, float hi)
     return p;
 }
 __device__ __forceinline__ Pk<double> pk_make(double lo, double hi) { return Pk<double>{lo, hi}; }
+// a pair whose halves the compiler must treat as unrelated (no scalar-broadcast operand form)
+__device__ __forceinline__ Pk<float> pk_pair(float lo, float hi)
+{
+    Pk<float> p;
+    asm volatile("mov.b64 %0, {%1, %2};" : "=l"(p.r) : "f"(lo), "f"(hi));
+    return p;
+}
+__device__ __forceinline__ Pk<double> pk_pair(double lo, double hi) { return Pk<double>{lo, hi}; }
 __device__ __forceinline__ float pk_lo(Pk<float> p)
 {
     float lo, hi;
@@ -212,6 +220,32 @@ __device__ __forceinline__ void sts1(uint32_t a, T v)
     const T o[1] = {v};
     sts<T, 1>(a, o);
 }
+
+// read-only global load that stays where it is written (the compiler may not hoist it: a load issued long
+// before its use keeps a scoreboard busy across loop back edges)
+__device__ __forceinline__ float ldg_here(const float* p)
+{
+    float v;
+    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ double ldg_here(const double* p)
+{
+    double v;
+    asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+
+// asynchronous copy of one element global -> shared (LDGSTS): no register, no scoreboard; wait with cp_async_wait()
+__device__ __forceinline__ void cp_async_elem(uint32_t dst, const float* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_elem(uint32_t dst, const double* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // rho[k] = (T) racc[k]
 template <typename T>
