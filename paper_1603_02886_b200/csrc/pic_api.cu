@@ -9,6 +9,14 @@ namespace pic {
 static thread_local int g_launches = 0;
 void count_launch(int n) { g_launches += n; }
 
+int sm_count()
+{
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+        return 148;
+    return sms;
+}
+
 static thread_local cudaEvent_t g_events[PIC_NUM_PHASES];
 static thread_local int g_num_events = 0;
 void mark_phase(int phase, cudaStream_t st)
@@ -200,22 +208,23 @@ int pic_step(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
         }
         if (in->w != o.w) PIC_CUDA_OK(cudaMemcpyAsync(o.w, in->w, s * (size_t)in->n, cudaMemcpyDeviceToDevice, st));
     }
-    const int order_state = do_sort ? PIC_ORDER_SORTED : (cell_offsets ? PIC_ORDER_STALE : PIC_ORDER_UNSORTED);
     if (!do_sort) mark_phase(PIC_PHASE_BEGIN, st);
-    if (order_state == PIC_ORDER_SORTED) {       // one fused kernel over the sorted particles
-        rc = launch_fused(*grid, *in, o, perm, cell_offsets, rho, E, dt, qm, sws.racc, st);
+    if (do_sort) {                               // one fused kernel over the sorted particles
+        rc = launch_fused(*grid, *in, o, perm, sws, rho, E, dt, qm, st);
         mark_phase(PIC_PHASE_PUSH, st);
         return rc;
     }
-    if (order_state == PIC_ORDER_STALE && in->n > 0) {
+    if (cell_offsets && in->n > 0) {
+        // the order of an earlier sort: the same kernel in place.  It finds the runs of equal cell key itself
+        // (cell_offsets is not read), so the result is exact however far the particles have drifted
         if (!aligned16(cell_offsets)) return PIC_ERR_INVALID_ARG;
-        rc = launch_stale_step(*grid, o, cell_offsets, rho, E, dt, qm, sws.racc, sws.gate, st);
+        rc = launch_fused(*grid, o, o, nullptr, sws, rho, E, dt, qm, st);
         mark_phase(PIC_PHASE_PUSH, st);
         return rc;
     }
-    if ((rc = launch_deposit(*grid, o, order_state, cell_offsets, rho, sws.racc, st)) != PIC_OK) return rc;
+    if ((rc = launch_deposit(*grid, o, PIC_ORDER_UNSORTED, nullptr, rho, sws.racc, st)) != PIC_OK) return rc;
     mark_phase(PIC_PHASE_DEPOSIT, st);
-    rc = launch_push(*grid, o, order_state, cell_offsets, E, dt, qm, st);
+    rc = launch_push(*grid, o, PIC_ORDER_UNSORTED, nullptr, E, dt, qm, st);
     mark_phase(PIC_PHASE_PUSH, st);
     return rc;
 }

@@ -142,6 +142,8 @@ __device__ __forceinline__ T wrap_periodic(T x, T L, T inv_L)
         if ((expr) != cudaSuccess) return PIC_ERR_CUDA; \
     } while (0)
 
+// multiprocessors of the current device (grids of the grid-stride kernels are sized from it)
+int sm_count();
 // thread-local launch counter behind pic_last_launch_count()
 void count_launch(int n = 1);
 // records the caller's event for `phase` on `st` if pic_set_phase_events() installed one
@@ -167,7 +169,9 @@ struct SortWs {
     uint32_t* scan_status;   // [2][scan tiles]
     uint32_t* cls_status;    // [scan tiles of the classify tiles]
     uint32_t* counters;      // [64] tile tickets, number of movers, hint flag  (... to here)
-    uint32_t* gate;          // one word of counters: result of launch_offsets_check (0 = usable)
+    uint32_t* gate;          // one word of counters: 1 = more than half of the particles are movers (set by the sort)
+    uint32_t* stray_count;   // one word of counters: particles the step kernel has set aside (zeroed with the counters)
+    uint32_t* stray_list;    // [N] their slots (= idx[0]: free once perm is written)
     double* racc;            // [C] double accumulation grid of the deposit (not in the zero region)
     void* zero_begin;        // region that must be zero before a sort
     size_t zero_bytes;
@@ -185,23 +189,20 @@ int launch_deposit(const pic_grid_t& g, const pic_particles_t& p, int order_stat
                    const int32_t* cell_offsets, void* rho, double* racc, cudaStream_t st);
 int launch_push(const pic_grid_t& g, pic_particles_t& p, int order_state, const int32_t* cell_offsets,
                 const void* const E[3], double dt, double qm, cudaStream_t st);
-// *gate = 0 if cell_offsets can be walked cell by cell (off[0] = 0, off[C] = n, non-decreasing), else 1
-int launch_offsets_check(const pic_grid_t& g, const int32_t* cell_offsets, int64_t n, uint32_t* gate, cudaStream_t st);
 // the threads-on-particles kernels alone; they run only if *gate == want (gate may be NULL); racc is not zeroed
 int launch_deposit_particles(const pic_grid_t& g, const pic_particles_t& p, double* racc, const uint32_t* gate,
                              uint32_t want, cudaStream_t st);
 int launch_push_particles(const pic_grid_t& g, pic_particles_t& p, const void* const E[3], double dt, double qm,
                           const uint32_t* gate, uint32_t want, cudaStream_t st);
-// pic_step(do_sort = 0) on particles that were sorted some steps ago: in place, cell by cell along the
-// old cell_offsets, the particles that left their cell since taken one by one (any-order fallback if the
-// offsets fail the check)
-int launch_stale_step(const pic_grid_t& g, pic_particles_t& p, const int32_t* cell_offsets, void* rho,
-                      const void* const E[3], double dt, double qm, double* racc, uint32_t* gate, cudaStream_t st);
-// deposit at x(t) + gather + accel + push in ONE kernel over particles sorted by cell: in place on
-// p (perm == NULL), or reading particle perm[j] of src and writing slot j of p (the sort's reorder
-// fused into the same pass)
+// deposit at x(t) + gather + accel + push in ONE kernel over particles in cell order: in place on p
+// (perm == NULL), or reading particle perm[j] of src and writing slot j of p (the sort's reorder fused into
+// the same pass).  With perm, *ws.gate (written by the sort: 1 = most particles move) chooses on the device
+// between that one pass and reorder-then-in-place; without perm, *ws.stray_count is zeroed here.  Lone
+// particles go through ws.stray_list to a threads-on-particles kernel.
 int launch_fused(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
-                 const int32_t* cell_offsets, void* rho, const void* const E[3], double dt, double qm, double* racc,
-                 cudaStream_t st);
+                 const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st);
+// out_a[j] = in_a[perm[j]] for every attribute; runs only if *gate == want (gate may be NULL)
+int launch_reorder(const pic_grid_t& g, const pic_particles_t& in, const pic_particles_t& out, const int32_t* perm,
+                   const uint32_t* gate, uint32_t want, cudaStream_t st);
 
 }  // namespace pic

@@ -4,9 +4,9 @@
 //
 // k_deposit_particles is the paper's collision-resolving "threads on particles" algorithm
 // (setrho 3.3.4): one thread per particle, (p+1)^d atomic adds to the grid.
-// It is correct for ANY particle order and is the path for PIC_ORDER_UNSORTED / STALE input.
-// Particles sorted by cell (PIC_ORDER_SORTED) go through k_rows (pic_rows.cuh).
-#include "pic_rows.cuh"
+// It is correct for ANY particle order and is the path for PIC_ORDER_UNSORTED input.
+// Particles in cell order (PIC_ORDER_SORTED / STALE) go through k_runs (pic_runs.cuh).
+#include "pic_runs.cuh"
 
 namespace pic {
 
@@ -69,8 +69,8 @@ static int deposit_impl(const pic_grid_t& g, const pic_particles_t& p, int order
     if (!racc) return PIC_ERR_WORKSPACE;
     PIC_CUDA_OK(cudaMemsetAsync(racc, 0, sizeof(double) * (size_t)C, st));
     if (p.n > 0) {
-        if (order_state == PIC_ORDER_SORTED) {
-            int rc = launch_rows<T, D, P, kModeDeposit, false>(g, p, p, nullptr, cell_offsets, nullptr, racc, 0.0, 0.0, st);
+        if (order_state != PIC_ORDER_UNSORTED) {       // cell order, exact or stale: runs of equal key (cell_offsets is not read)
+            int rc = launch_runs<T, D, P, kModeDeposit, false>(g, p, p, nullptr, nullptr, racc, 0.0, 0.0, st);
             if (rc != PIC_OK) return rc;
         } else {
             k_deposit_particles<T, D, P><<<(unsigned)((p.n + 255) / 256), 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g),

@@ -8,7 +8,7 @@
 // and counts 6 loads + 3 stores for each; fused they are
 // 2d loads + 2d stores per particle.  k_push_particles reads E through the read-only path
 // ("scattered reads through read-only data cache") and is correct for any order.
-#include "pic_rows.cuh"
+#include "pic_runs.cuh"
 
 namespace pic {
 
@@ -65,8 +65,8 @@ static int push_impl(const pic_grid_t& g, pic_particles_t& p, int order_state, c
                      const void* const E[3], double dt, double qm, cudaStream_t st)
 {
     if (p.n > 0) {
-        if (order_state == PIC_ORDER_SORTED)
-            return launch_rows<T, D, P, kModePush, false>(g, p, p, nullptr, cell_offsets, E, nullptr, dt, qm, st);
+        if (order_state != PIC_ORDER_UNSORTED)         // cell order, exact or stale: runs of equal key (cell_offsets is not read)
+            return launch_runs<T, D, P, kModePush, false>(g, p, p, nullptr, E, nullptr, dt, qm, st);
         FieldP<T> f;
         for (int c = 0; c < 3; ++c) f.E[c] = c < D ? (const T*)E[c] : nullptr;
         k_push_particles<T, D, P><<<(unsigned)((p.n + 255) / 256), 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), f, p.n,

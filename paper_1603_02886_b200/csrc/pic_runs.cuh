@@ -50,10 +50,14 @@ namespace pic {
 #ifndef PIC_RUNS_WR
 #define PIC_RUNS_WR 2048        // slots per warp
 #endif
+#ifndef PIC_RUNS_UNROLL
+#define PIC_RUNS_UNROLL 2       // units of phase N in flight
+#endif
 #ifndef PIC_RUNS_WARPS
 #define PIC_RUNS_WARPS 1        // warps per block (warps are independent)
 #endif
 constexpr int kRunsWarps = PIC_RUNS_WARPS;
+constexpr int kRunsUnroll = PIC_RUNS_UNROLL;
 constexpr int kRunsThreads = 32 * kRunsWarps;
 
 template <typename T, int D, int P, int G_>
@@ -92,6 +96,13 @@ constexpr int runs_min_blocks()
 {
     return (sizeof(T) == 4 ? PIC_RUNS_MINW32 : PIC_RUNS_MINW64) / PIC_RUNS_WARPS;
 }
+// register budget of k_runs: a cap per thread (fp32: 136 registers = 15 warps per SM; at 128 ptxas spills a
+// prefetched particle attribute, which exposes the whole memory latency), else a resident-block target
+#ifdef PIC_RUNS_MAXREG32
+#define PIC_RUNS_BOUNDS(T) __maxnreg__(sizeof(T) == 4 ? PIC_RUNS_MAXREG32 : 255)
+#else
+#define PIC_RUNS_BOUNDS(T) __launch_bounds__(kRunsThreads, (runs_min_blocks<T>()))
+#endif
 
 // v[s] <- v[(s - rho) mod S]: the weight of stencil column i goes to column slot (i + rho) mod S
 template <typename T, int S>
@@ -108,10 +119,67 @@ __device__ __forceinline__ void rotate_slots(T (&v)[S], int rho)
     }
 }
 
-template <typename T, int D, int P, int MODE, bool VIA_PERM, int G_>
-__global__ void __launch_bounds__(kRunsThreads, (runs_min_blocks<T>()))
+// The STRAYS k_runs has set aside (particles whose key differs from both neighbours': drifted particles of a
+// stale order, one-particle cells), one thread each: "threads on particles" with global reductions (setrho
+// 3.3.4; accel through the read-only path).  list[0 .. *count) holds their slots
+// in p, where k_runs has left them un-advanced.
+template <typename T, int D, int P, int MODE>
+__global__ void __launch_bounds__(128) k_strays(PartP<T> p, GridP<T> g, FieldP<T> f, const uint32_t* __restrict__ list,
+                                                const uint32_t* __restrict__ count, double* __restrict__ racc, T dt, T qmdt)
+{
+    const uint32_t m = *count;
+    for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < m; t += gridDim.x * blockDim.x) {
+        const uint32_t j = list[t];
+        T x[D], v[D], e[D];
+        int first[3] = {0, 0, 0};
+        T wt[3][P + 1];
+#pragma unroll
+        for (int c = 0; c < D; ++c) {
+            x[c] = p.x[c][j];
+            e[c] = (T)0;
+            const T tt = grid_coord(x[c], g.h[c], g.inv_h[c], g.hmul);
+            spline_weights<T, P>(tt, cell_index(tt, g.n[c]), first[c], wt[c]);
+        }
+        const T q = (MODE & kModeDeposit) ? p.w[j] * g.inv_vol : (T)0;
+        constexpr int PZ = (D == 3) ? P : 0;
+#pragma unroll
+        for (int cz = 0; cz <= PZ; ++cz) {
+            const int jz = (D == 3) ? fold(first[2] + cz, g.n[2]) : 0;
+            const T wz = (D == 3) ? wt[2][cz] : (T)1;
+#pragma unroll
+            for (int b = 0; b <= P; ++b) {
+                const int jy = fold(first[1] + b, g.n[1]);
+                const T wyz = wz * wt[1][b];
+                const int row = g.n[0] * (jy + g.n[1] * jz);
+#pragma unroll
+                for (int a = 0; a <= P; ++a) {
+                    const int at = row + fold(first[0] + a, g.n[0]);
+                    const T wgt = wyz * wt[0][a];
+                    if constexpr ((MODE & kModeDeposit) != 0) atomicAdd(&racc[at], (double)(q * wgt));
+                    if constexpr ((MODE & kModePush) != 0) {
+#pragma unroll
+                        for (int c = 0; c < D; ++c) e[c] += wgt * __ldg(f.E[c] + at);
+                    }
+                }
+            }
+        }
+        if constexpr ((MODE & kModePush) != 0) {
+#pragma unroll
+            for (int c = 0; c < D; ++c) {
+                v[c] = p.v[c][j] + qmdt * e[c];
+                p.v[c][j] = v[c];
+                p.x[c][j] = wrap_periodic(x[c] + dt * v[c], g.L[c], g.inv_L[c]);
+            }
+        }
+    }
+}
+
+// STRAYS: lone particles are set aside in stray_list for k_strays (used where the order may be stale)
+template <typename T, int D, int P, int MODE, bool VIA_PERM, int G_, bool STRAYS>
+__global__ void PIC_RUNS_BOUNDS(T)
 k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g, FieldP<T> f, int64_t n,
-       double* __restrict__ racc, T dt, T qmdt, const uint32_t* __restrict__ gate, uint32_t want)
+       double* __restrict__ racc, T dt, T qmdt, const uint32_t* __restrict__ gate, uint32_t want,
+       uint32_t* __restrict__ stray_list, uint32_t* __restrict__ stray_count)
 {
     using SH = RunsShape<T, D, P, G_>;
     if (gate && *gate != want) return;                // the other arm of a device-side choice runs instead
@@ -315,26 +383,66 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
 
         // ---- phase W: lane = slot
         int key = -1, c0, c1, c2 = 0;
-        {
+        int idx = lane, nrec = nb;                    // this lane's record index, records in the batch
+        bool lonely = false;
+        auto write_record = [&]() {
             T w1[S], w2[S], w3[SZ];
-            c0 = cell_weights<T, P>(px[0], g.h[0], g.inv_h[0], g.hmul, g.n[0], w1);
-            c1 = cell_weights<T, P>(px[1], g.h[1], g.inv_h[1], g.hmul, g.n[1], w2);
-            if constexpr (D == 3) c2 = cell_weights<T, P>(px[2], g.h[2], g.inv_h[2], g.hmul, g.n[2], w3);
-            if (valid) key = c0 + g.n[0] * (c1 + g.n[1] * c2);
-            rotate_slots<T, S>(w1, c0 - sh);          // x weights by column slot
-            const uint32_t rec = a_rec + (uint32_t)(lane * RECS) * B;
+            const int cx = cell_weights<T, P>(px[0], g.h[0], g.inv_h[0], g.hmul, g.n[0], w1);
+            const int cy = cell_weights<T, P>(px[1], g.h[1], g.inv_h[1], g.hmul, g.n[1], w2);
+            int cz = 0;
+            if constexpr (D == 3) cz = cell_weights<T, P>(px[2], g.h[2], g.inv_h[2], g.hmul, g.n[2], w3);
+            if constexpr (!STRAYS) {
+                c0 = cx; c1 = cy; c2 = cz;
+                if (valid) key = c0 + g.n[0] * (c1 + g.n[1] * c2);
+            }
+            rotate_slots<T, S>(w1, cx - sh);          // x weights by column slot
+            const uint32_t rec = a_rec + (uint32_t)(idx * RECS) * B;
             sts<T, S>(rec, w1);
             sts<T, S>(rec + S * B, w2);
             if constexpr (D == 3) sts<T, S>(rec + 2 * S * B, w3);
-            if constexpr (DEP) sts1<T>(a_q + (uint32_t)lane * B, valid ? pw * g.inv_vol : (T)0);
+            if constexpr (DEP) sts1<T>(a_q + (uint32_t)idx * B, (valid && !lonely) ? pw * g.inv_vol : (T)0);
+        };
+        if constexpr (STRAYS) {
+            c0 = cell_index(grid_coord(px[0], g.h[0], g.inv_h[0], g.hmul), g.n[0]);
+            c1 = cell_index(grid_coord(px[1], g.h[1], g.inv_h[1], g.hmul), g.n[1]);
+            if constexpr (D == 3) c2 = cell_index(grid_coord(px[2], g.h[2], g.inv_h[2], g.hmul), g.n[2]);
+            if (valid) key = c0 + g.n[0] * (c1 + g.n[1] * c2);
+            // a particle whose key differs from both neighbours' is a STRAY: it does not break the run around it but
+            // is set aside for k_strays.  The others are the RECORDS of the batch, in order.
+            const int kleft = __shfl_up_sync(FULL, key, 1), kright = __shfl_down_sync(FULL, key, 1);
+            lonely = valid && key != (lane == 0 ? cur : kleft) && (lane == nb - 1 || key != kright);
+            const unsigned strays = __ballot_sync(FULL, lonely);
+            if (strays) {                             // warp-uniform; rare in cell order: compact the records
+                const unsigned keep = (nb == 32 ? FULL : ((1u << nb) - 1u)) & ~strays, below = (1u << lane) - 1u;
+                nrec = __popc(keep);
+                idx = lonely ? nrec + __popc(strays & below) : __popc(keep & below);  // (strays: unused records behind)
+                uint32_t at = 0;
+                if (lane == 0) at = atomicAdd(stray_count, (uint32_t)__popc(strays));
+                at = __shfl_sync(FULL, at, 0);
+                if (lonely) stray_list[at + __popc(strays & below)] = (uint32_t)(jl + b0);
+                write_record();                       // (own cell: before the keys are permuted)
+                const uint32_t tmp = a_part;          // the partial-field buffer is free here: 4 ints per record
+                if (valid && !lonely)
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" :: "r"(tmp + idx * 16), "r"(key), "r"(c0), "r"(c1), "r"(c2) : "memory");
+                __syncwarp();
+                key = -1;
+                if (lane < nrec)
+                    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(key), "=r"(c0), "=r"(c1), "=r"(c2) : "r"(tmp + lane * 16));
+                __syncwarp();
+            } else {
+                write_record();
+            }
+        } else {
+            write_record();
         }
+        // key, c0, c1, c2 now belong to record `lane`
         const int kprev = __shfl_up_sync(FULL, key, 1);
-        const unsigned heads = __ballot_sync(FULL, valid && key != (lane == 0 ? cur : kprev));
+        const unsigned heads = __ballot_sync(FULL, lane < nrec && key != (lane == 0 ? cur : kprev));
         __syncwarp();
 
         // ---- phase N: lanes on stencil rows, run by run
         int pos = 0;
-        while (pos < nb) {
+        while (pos < nrec) {
             const bool head = (heads >> pos) & 1u;
             if (head) {                               // the key changes here
                 const bool had = cur >= 0;
@@ -351,9 +459,9 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
                 flush_all();
             }
             const unsigned above = (pos < 31) ? (heads & ~((2u << pos) - 1u)) : 0u;
-            const int end = above ? __ffs(above) - 1 : nb;
+            const int end = above ? __ffs(above) - 1 : nrec;
             // the groups take records pos.., one each; a group beyond the end repeats the last record with q = 0
-#pragma unroll 2
+#pragma unroll (STRAYS ? 1 : kRunsUnroll)
             for (int u = pos; u < end; u += NG) {
                 const bool live = u + grp < end;
                 const int r = live ? u + grp : end - 1;
@@ -404,12 +512,12 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
         // ---- phase P: lane = slot again: accel + push + store
         if (valid) {
             const int64_t j = jl + b0;
-            if constexpr (PUSH) {
+            if (PUSH && !lonely) {
                 bool inside = true;
 #pragma unroll
                 for (int c = 0; c < D; ++c) {
                     T pe[G];
-                    lds<T, G>(a_part + (uint32_t)((lane * D + c) * G) * B, pe);
+                    lds<T, G>(a_part + (uint32_t)((idx * D + c) * G) * B, pe);
                     T e = pe[0];
 #pragma unroll
                     for (int q = 1; q < G; ++q) e += pe[q];
@@ -422,7 +530,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
                     for (int c = 0; c < D; ++c) px[c] = wrap_periodic(px[c], g.L[c], g.inv_L[c]);
                 }
             }
-            if constexpr (PUSH || VIA_PERM) {
+            if ((PUSH && !lonely) || VIA_PERM) {
 #pragma unroll
                 for (int c = 0; c < D; ++c) { dst.x[c][j] = px[c]; dst.v[c][j] = pv[c]; }
                 if constexpr (VIA_PERM) dst.w[j] = pw;
@@ -435,24 +543,49 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
 
 // launch k_runs over n particles.  VIA_PERM: particle perm[j] of src -> slot j of dst; otherwise in place
 // on dst.  racc = double accumulation grid of the deposit.  The kernel runs only if *gate == want (gate
-// may be NULL).
+// may be NULL).  stray_list / stray_count (both or neither; *stray_count zeroed by the caller): lone particles
+// are set aside there for launch_strays instead of breaking the run they sit in.
 template <typename T, int D, int P, int MODE, bool VIA_PERM>
 inline int launch_runs(const pic_grid_t& g, const pic_particles_t& src, const pic_particles_t& dst,
                        const int32_t* perm, const void* const E[3], double* racc, double dt, double qm,
-                       cudaStream_t st, const uint32_t* gate = nullptr, uint32_t want = 0)
+                       cudaStream_t st, const uint32_t* gate = nullptr, uint32_t want = 0,
+                       uint32_t* stray_list = nullptr, uint32_t* stray_count = nullptr)
 {
     if (dst.n <= 0) return PIC_OK;
     constexpr int GP = sizeof(T) == 4 ? PIC_RUNS_G32 : PIC_RUNS_G64;
     using SH = RunsShape<T, D, P, GP>;
     FieldP<T> f;
     for (int c = 0; c < 3; ++c) f.E[c] = (E && c < D) ? (const T*)E[c] : nullptr;
-    auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP>;
     constexpr size_t smem = SH::bytes;
     static_assert(smem <= 48 * 1024, "k_runs relies on the default dynamic shared memory limit");
     constexpr int64_t per_block = (int64_t)SH::WR * kRunsWarps;
     const unsigned blocks = (unsigned)((dst.n + per_block - 1) / per_block);
+    if (stray_list && stray_count) {
+        auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, true>;
+        kern<<<blocks, kRunsThreads, smem, st>>>(make_partp<T>(VIA_PERM ? src : dst), make_partp<T>(dst), perm,
+                                                make_gridp<T>(g), f, dst.n, racc, (T)dt, (T)(qm * dt), gate, want,
+                                                stray_list, stray_count);
+        count_launch();
+        return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+    }
+    auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, false>;
     kern<<<blocks, kRunsThreads, smem, st>>>(make_partp<T>(VIA_PERM ? src : dst), make_partp<T>(dst), perm,
-                                            make_gridp<T>(g), f, dst.n, racc, (T)dt, (T)(qm * dt), gate, want);
+                                            make_gridp<T>(g), f, dst.n, racc, (T)dt, (T)(qm * dt), gate, want,
+                                            stray_list, stray_count);
+    count_launch();
+    return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+}
+
+// the particles k_runs has set aside, in place on p
+template <typename T, int D, int P, int MODE>
+inline int launch_strays(const pic_grid_t& g, const pic_particles_t& p, const void* const E[3], double* racc, double dt,
+                         double qm, const uint32_t* stray_list, const uint32_t* stray_count, int sms, cudaStream_t st)
+{
+    if (p.n <= 0) return PIC_OK;
+    FieldP<T> f;
+    for (int c = 0; c < 3; ++c) f.E[c] = (E && c < D) ? (const T*)E[c] : nullptr;
+    k_strays<T, D, P, MODE><<<(unsigned)(sms * 8), 128, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), f, stray_list, stray_count,
+                                                              racc, (T)dt, (T)(qm * dt));
     count_launch();
     return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }

@@ -61,7 +61,7 @@ constexpr int kClsWarps = kClsThreads / 32;
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagPrefix = 2u << 30, kValMask = (1u << 30) - 1;
 
 // slots of SortWs::counters
-enum { kCtrScanA = 0, kCtrScanB = 1, kCtrCls = 2, kCtrRadix = 3 /* .. +kMaxPasses */, kCtrMovers = 8, kCtrHintBad = 9, kCtrGate = 16 };
+enum { kCtrScanA = 0, kCtrScanB = 1, kCtrCls = 2, kCtrRadix = 3 /* .. +kMaxPasses */, kCtrMovers = 8, kCtrHintBad = 9, kCtrGate = 16, kCtrStrays = 17 };
 
 __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p)
 {
@@ -109,27 +109,6 @@ __global__ void __launch_bounds__(256) k_hint_check(const int32_t* __restrict__ 
     bool bad = a < 0 || (int64_t)a > n;
     if (k < C) bad = bad || hint[k + 1] < a;
     if (bad) counters[kCtrHintBad] = 1u;
-}
-
-// *gate = 1 unless off[0] = 0 <= off[1] <= ... <= off[C] = n (the caller zeroes *gate)
-__global__ void __launch_bounds__(256) k_offsets_check(const int32_t* __restrict__ off, int C, int64_t n, uint32_t* gate)
-{
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k > C) return;
-    const int32_t a = off[k];
-    bool bad = a < 0 || (int64_t)a > n || (k == 0 && a != 0) || (k == C && (int64_t)a != n);
-    if (k < C) bad = bad || off[k + 1] < a;
-    if (bad) *gate = 1u;
-}
-
-int launch_offsets_check(const pic_grid_t& g, const int32_t* cell_offsets, int64_t n, uint32_t* gate, cudaStream_t st)
-{
-    int64_t C = 1;
-    for (int c = 0; c < g.dim; ++c) C *= g.n[c];
-    PIC_CUDA_OK(cudaMemsetAsync(gate, 0, sizeof(uint32_t), st));
-    k_offsets_check<<<(unsigned)((C + 1 + 255) / 256), 256, 0, st>>>(cell_offsets, (int)C, n, gate);
-    count_launch();
-    return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
 
 // ----------------------------------------------------------------------------- keys, histograms, stayer/mover split
@@ -352,6 +331,7 @@ k_movers_place(const uint32_t* __restrict__ stage_key, const uint32_t* __restric
     if (tile == ntiles - 1 && tid == 0) {                // total number of movers, sentinel word
         const uint32_t total = (uint32_t)tile_base[ntiles];
         counters[kCtrMovers] = total;
+        counters[kCtrGate] = (2 * (int64_t)total > n) ? 1u : 0u;      // most particles move: reorder before the step kernel
         mask[nwords] = 0u;
         mprefix[nwords] = total;
     }
@@ -652,18 +632,20 @@ k_perm_stayers(const uint32_t* __restrict__ pkey, const int32_t* __restrict__ ce
 // ----------------------------------------------------------------------------- reorder
 // a4: out_a[j] = in_a[perm[j]] for all attributes, bit for bit; coalesced writes, gathered reads.
 template <typename T, int D>
-__global__ void __launch_bounds__(256) k_reorder(PartP<T> in, PartP<T> out, const int32_t* __restrict__ perm, int64_t n)
+__global__ void __launch_bounds__(256) k_reorder(PartP<T> in, PartP<T> out, const int32_t* __restrict__ perm, int64_t n,
+                                                 const uint32_t* __restrict__ gate, uint32_t want)
 {
-    int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n) return;
-    const int64_t i = perm[j];
-    T x[D], v[D];
+    if (gate && *gate != want) return;
+    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = perm[j];
+        T x[D], v[D];
 #pragma unroll
-    for (int c = 0; c < D; ++c) { x[c] = in.x[c][i]; v[c] = in.v[c][i]; }
-    T w = in.w[i];
+        for (int c = 0; c < D; ++c) { x[c] = in.x[c][i]; v[c] = in.v[c][i]; }
+        const T w = in.w[i];
 #pragma unroll
-    for (int c = 0; c < D; ++c) { out.x[c][j] = x[c]; out.v[c][j] = v[c]; }
-    out.w[j] = w;
+        for (int c = 0; c < D; ++c) { out.x[c][j] = x[c]; out.v[c][j] = v[c]; }
+        out.w[j] = w;
+    }
 }
 
 // ----------------------------------------------------------------------------- host side
@@ -760,6 +742,8 @@ int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, Sor
     o.cls_status = (uint32_t*)(b + L.cls_status);
     o.counters = (uint32_t*)(b + L.counters);
     o.gate = o.counters + kCtrGate;
+    o.stray_count = o.counters + kCtrStrays;
+    o.stray_list = o.idx[0];
     o.zero_begin = b + L.zero_begin;
     o.zero_bytes = L.zero_end - L.zero_begin;
     o.racc = (double*)(b + L.racc);
@@ -804,7 +788,7 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
                                                                         ws.digit_hist, ws.passes, ws.bits_per_pass);
         k_scan_digits<<<ws.passes, kRadix, 0, st>>>(ws.digit_hist);
         const int64_t pass_stride = ws.radix_tiles * kRadix;
-        k_zero_lookback<<<148 * 4, 256, 0, st>>>(ws.lookback, ws.counters, ws.passes, pass_stride);
+        k_zero_lookback<<<sm_count() * 4, 256, 0, st>>>(ws.lookback, ws.counters, ws.passes, pass_stride);
         count_launch(3);
         mark_phase(PIC_PHASE_SCAN, st);
         int src = 0;
@@ -821,14 +805,14 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
         mark_phase(PIC_PHASE_RADIX, st);
         k_cell_base<<<(unsigned)((C + 255) / 256), 256, 0, st>>>(cell_offsets, ws.old_off, ws.mover_lo, ws.mask, ws.mprefix,
                                                                  ws.cell_base, C, ws.counters);
-        k_perm_movers<<<148 * 8, 256, 0, st>>>(ws.keys[src], ws.idx[src], cell_offsets, ws.mover_off, ws.old_off, perm,
+        k_perm_movers<<<sm_count() * 8, 256, 0, st>>>(ws.keys[src], ws.idx[src], cell_offsets, ws.mover_off, ws.old_off, perm,
                                               ws.counters);
         k_perm_stayers<<<(unsigned)((n + 256 * kStayIPT - 1) / (256 * kStayIPT)), 256, 0, st>>>(
             ws.pkey, ws.cell_base, ws.mask, ws.mprefix, perm, (int)n, ws.counters);
         count_launch(3);
     }
     mark_phase(PIC_PHASE_REORDER, st);
-    return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+    return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
 
 template <typename T, int D>
@@ -838,11 +822,27 @@ static int sort_impl(const pic_grid_t& g, const pic_particles_t& in, pic_particl
     int rc = sort_keys_perm<T, D>(g, in, perm, cell_offsets, ws, st);
     if (rc != PIC_OK) return rc;
     const int64_t n = in.n;
-    if (n > 0 && reorder) {
-        k_reorder<T, D><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(make_partp<T>(in), make_partp<T>(out), perm, n);
-        count_launch();
+    if (n > 0 && reorder) return launch_reorder(g, in, out, perm, nullptr, 0u, st);
+    return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+}
+
+int launch_reorder(const pic_grid_t& g, const pic_particles_t& in, const pic_particles_t& out, const int32_t* perm,
+                   const uint32_t* gate, uint32_t want, cudaStream_t st)
+{
+    const int64_t n = in.n;
+    if (n <= 0) return PIC_OK;
+    // a grid-stride loop over a fixed grid (8 blocks per multiprocessor): cheap to launch when the gate says no
+    const int64_t want_blocks = (n + 255) / 256, cap = (int64_t)sm_count() * 8;
+    const unsigned blocks = (unsigned)(want_blocks < cap ? want_blocks : cap);
+    if (g.dtype == PIC_F32) {
+        if (g.dim == 2) k_reorder<float, 2><<<blocks, 256, 0, st>>>(make_partp<float>(in), make_partp<float>(out), perm, n, gate, want);
+        else k_reorder<float, 3><<<blocks, 256, 0, st>>>(make_partp<float>(in), make_partp<float>(out), perm, n, gate, want);
+    } else {
+        if (g.dim == 2) k_reorder<double, 2><<<blocks, 256, 0, st>>>(make_partp<double>(in), make_partp<double>(out), perm, n, gate, want);
+        else k_reorder<double, 3><<<blocks, 256, 0, st>>>(make_partp<double>(in), make_partp<double>(out), perm, n, gate, want);
     }
-    return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+    count_launch();
+    return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
 
 int launch_sort(const pic_grid_t& g, const pic_particles_t& in, pic_particles_t& out, int32_t* perm,
