@@ -24,6 +24,7 @@ struct GridP {
     T inv_L[3];
     T inv_vol;       // 1 / prod h
     int hmul;        // 1: every h is a power of two, x*inv_h == x/h bit for bit
+    double Ld[3];    // box length in double (advance_wrap)
 };
 
 template <typename T>
@@ -40,6 +41,7 @@ inline GridP<T> make_gridp(const pic_grid_t& g)
         p.inv_h[c] = (T)1 / p.h[c];
         double L = (double)p.n[c] * h;
         p.L[c] = (T)L;
+        p.Ld[c] = L;
         p.inv_L[c] = (T)(1.0 / L);
         if (on) {
             vol *= h;
@@ -137,6 +139,21 @@ __device__ __forceinline__ T wrap_periodic(T x, T L, T inv_L)
     return x;
 }
 
+// A particle that leaves [0, L) in this step: accel and push are redone in double precision, wrapped and
+// rounded once, as O4 states them.  (In the storage precision the sum x + dt v loses the low bits of x as soon
+// as the particle crosses several boxes; inside the box the plain storage-precision update is within half an
+// ulp of L of this.)  Out of line: the call is rare.
+template <typename T>
+__device__ __noinline__ T advance_wrap(T x_old, T v_old, T e, double dt, double qmdt, double L)
+{
+    const double vn = (double)v_old + qmdt * (double)e;
+    double xn = (double)x_old + dt * vn;
+    xn -= L * floor(xn / L);
+    T xs = (T)xn;
+    if (!(xs >= (T)0 && xs < (T)L)) xs = (T)0;
+    return xs;
+}
+
 #define PIC_CUDA_OK(expr)                          \
     do {                                           \
         if ((expr) != cudaSuccess) return PIC_ERR_CUDA; \
@@ -189,11 +206,6 @@ int launch_deposit(const pic_grid_t& g, const pic_particles_t& p, int order_stat
                    const int32_t* cell_offsets, void* rho, double* racc, cudaStream_t st);
 int launch_push(const pic_grid_t& g, pic_particles_t& p, int order_state, const int32_t* cell_offsets,
                 const void* const E[3], double dt, double qm, cudaStream_t st);
-// the threads-on-particles kernels alone; they run only if *gate == want (gate may be NULL); racc is not zeroed
-int launch_deposit_particles(const pic_grid_t& g, const pic_particles_t& p, double* racc, const uint32_t* gate,
-                             uint32_t want, cudaStream_t st);
-int launch_push_particles(const pic_grid_t& g, pic_particles_t& p, const void* const E[3], double dt, double qm,
-                          const uint32_t* gate, uint32_t want, cudaStream_t st);
 // deposit at x(t) + gather + accel + push in ONE kernel over particles in cell order: in place on p
 // (perm == NULL), or reading particle perm[j] of src and writing slot j of p (the sort's reorder fused into
 // the same pass).  With perm, *ws.gate (written by the sort: 1 = most particles move) chooses on the device

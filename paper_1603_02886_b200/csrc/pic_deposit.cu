@@ -11,10 +11,8 @@
 namespace pic {
 
 template <typename T, int D, int P>
-__global__ void __launch_bounds__(256) k_deposit_particles(PartP<T> p, GridP<T> g, int64_t n, double* __restrict__ rho,
-                                                           const uint32_t* __restrict__ gate, uint32_t want)
+__global__ void __launch_bounds__(256) k_deposit_particles(PartP<T> p, GridP<T> g, int64_t n, double* __restrict__ rho)
 {
-    if (gate && *gate != want) return;
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int first[3] = {0, 0, 0};
@@ -74,7 +72,7 @@ static int deposit_impl(const pic_grid_t& g, const pic_particles_t& p, int order
             if (rc != PIC_OK) return rc;
         } else {
             k_deposit_particles<T, D, P><<<(unsigned)((p.n + 255) / 256), 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g),
-                                                                                       p.n, racc, nullptr, 0u);
+                                                                                       p.n, racc);
             count_launch();
         }
     }
@@ -82,7 +80,7 @@ static int deposit_impl(const pic_grid_t& g, const pic_particles_t& p, int order
         k_round_rho<T><<<(unsigned)((C + 255) / 256), 256, 0, st>>>(racc, (T*)rho, C);
         count_launch();
     }
-    return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+    return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
 
 template <typename T, int D>
@@ -94,32 +92,6 @@ static int deposit_order(const pic_grid_t& g, const pic_particles_t& p, int orde
     case 2: return deposit_impl<T, D, 2>(g, p, order_state, cell_offsets, rho, racc, st);
     default: return deposit_impl<T, D, 3>(g, p, order_state, cell_offsets, rho, racc, st);
     }
-}
-
-// threads-on-particles deposit into racc (not zeroed here), run only if *gate == want (gate may be NULL)
-template <typename T, int D>
-static int deposit_particles_order(const pic_grid_t& g, const pic_particles_t& p, double* racc, const uint32_t* gate,
-                                   uint32_t want, cudaStream_t st)
-{
-    const unsigned blocks = (unsigned)((p.n + 255) / 256);
-    switch (g.order) {
-    case 1: k_deposit_particles<T, D, 1><<<blocks, 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), p.n, racc, gate, want); break;
-    case 2: k_deposit_particles<T, D, 2><<<blocks, 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), p.n, racc, gate, want); break;
-    default: k_deposit_particles<T, D, 3><<<blocks, 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), p.n, racc, gate, want); break;
-    }
-    count_launch();
-    return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
-}
-
-int launch_deposit_particles(const pic_grid_t& g, const pic_particles_t& p, double* racc, const uint32_t* gate,
-                             uint32_t want, cudaStream_t st)
-{
-    if (p.n <= 0) return PIC_OK;
-    if (g.dtype == PIC_F32)
-        return g.dim == 2 ? deposit_particles_order<float, 2>(g, p, racc, gate, want, st)
-                          : deposit_particles_order<float, 3>(g, p, racc, gate, want, st);
-    return g.dim == 2 ? deposit_particles_order<double, 2>(g, p, racc, gate, want, st)
-                      : deposit_particles_order<double, 3>(g, p, racc, gate, want, st);
 }
 
 int launch_deposit(const pic_grid_t& g, const pic_particles_t& p, int order_state, const int32_t* cell_offsets,

@@ -13,10 +13,9 @@
 namespace pic {
 
 template <typename T, int D, int P>
-__global__ void __launch_bounds__(256) k_push_particles(PartP<T> p, GridP<T> g, FieldP<T> f, int64_t n, T dt, T qmdt,
-                                                        const uint32_t* __restrict__ gate, uint32_t want)
+__global__ void __launch_bounds__(256) k_push_particles(PartP<T> p, GridP<T> g, FieldP<T> f, int64_t n, double dtd, double qmdtd)
 {
-    if (gate && *gate != want) return;
+    const T dt = (T)dtd, qmdt = (T)qmdtd;
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int first[3] = {0, 0, 0};
@@ -53,10 +52,11 @@ __global__ void __launch_bounds__(256) k_push_particles(PartP<T> p, GridP<T> g, 
     }
 #pragma unroll
     for (int c = 0; c < D; ++c) {
-        v[c] += qmdt * e[c];
-        x[c] = wrap_periodic(x[c] + dt * v[c], g.L[c], g.inv_L[c]);
-        p.v[c][i] = v[c];
-        p.x[c][i] = x[c];
+        const T vn = v[c] + qmdt * e[c];
+        T xn = x[c] + dt * vn;
+        if (!(xn >= (T)0 && xn < g.L[c])) xn = advance_wrap<T>(x[c], v[c], e[c], dtd, qmdtd, g.Ld[c]);
+        p.v[c][i] = vn;
+        p.x[c][i] = xn;
     }
 }
 
@@ -70,10 +70,10 @@ static int push_impl(const pic_grid_t& g, pic_particles_t& p, int order_state, c
         FieldP<T> f;
         for (int c = 0; c < 3; ++c) f.E[c] = c < D ? (const T*)E[c] : nullptr;
         k_push_particles<T, D, P><<<(unsigned)((p.n + 255) / 256), 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), f, p.n,
-                                                                                (T)dt, (T)(qm * dt), nullptr, 0u);
+                                                                                dt, qm * dt);
         count_launch();
     }
-    return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+    return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
 
 template <typename T, int D>
@@ -85,35 +85,6 @@ static int push_order(const pic_grid_t& g, pic_particles_t& p, int order_state, 
     case 2: return push_impl<T, D, 2>(g, p, order_state, cell_offsets, E, dt, qm, st);
     default: return push_impl<T, D, 3>(g, p, order_state, cell_offsets, E, dt, qm, st);
     }
-}
-
-// threads-on-particles gather + push, run only if *gate == want (gate may be NULL)
-template <typename T, int D>
-static int push_particles_order(const pic_grid_t& g, pic_particles_t& p, const void* const E[3], double dt, double qm,
-                                const uint32_t* gate, uint32_t want, cudaStream_t st)
-{
-    FieldP<T> f;
-    for (int c = 0; c < 3; ++c) f.E[c] = c < D ? (const T*)E[c] : nullptr;
-    const unsigned blocks = (unsigned)((p.n + 255) / 256);
-    const T tdt = (T)dt, tq = (T)(qm * dt);
-    switch (g.order) {
-    case 1: k_push_particles<T, D, 1><<<blocks, 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), f, p.n, tdt, tq, gate, want); break;
-    case 2: k_push_particles<T, D, 2><<<blocks, 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), f, p.n, tdt, tq, gate, want); break;
-    default: k_push_particles<T, D, 3><<<blocks, 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), f, p.n, tdt, tq, gate, want); break;
-    }
-    count_launch();
-    return cudaGetLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
-}
-
-int launch_push_particles(const pic_grid_t& g, pic_particles_t& p, const void* const E[3], double dt, double qm,
-                          const uint32_t* gate, uint32_t want, cudaStream_t st)
-{
-    if (p.n <= 0) return PIC_OK;
-    if (g.dtype == PIC_F32)
-        return g.dim == 2 ? push_particles_order<float, 2>(g, p, E, dt, qm, gate, want, st)
-                          : push_particles_order<float, 3>(g, p, E, dt, qm, gate, want, st);
-    return g.dim == 2 ? push_particles_order<double, 2>(g, p, E, dt, qm, gate, want, st)
-                      : push_particles_order<double, 3>(g, p, E, dt, qm, gate, want, st);
 }
 
 int launch_push(const pic_grid_t& g, pic_particles_t& p, int order_state, const int32_t* cell_offsets,

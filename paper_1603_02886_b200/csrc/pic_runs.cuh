@@ -125,8 +125,9 @@ __device__ __forceinline__ void rotate_slots(T (&v)[S], int rho)
 // in p, where k_runs has left them un-advanced.
 template <typename T, int D, int P, int MODE>
 __global__ void __launch_bounds__(128) k_strays(PartP<T> p, GridP<T> g, FieldP<T> f, const uint32_t* __restrict__ list,
-                                                const uint32_t* __restrict__ count, double* __restrict__ racc, T dt, T qmdt)
+                                                const uint32_t* __restrict__ count, double* __restrict__ racc, double dtd, double qmdtd)
 {
+    const T dt = (T)dtd, qmdt = (T)qmdtd;
     const uint32_t m = *count;
     for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < m; t += gridDim.x * blockDim.x) {
         const uint32_t j = list[t];
@@ -166,9 +167,12 @@ __global__ void __launch_bounds__(128) k_strays(PartP<T> p, GridP<T> g, FieldP<T
         if constexpr ((MODE & kModePush) != 0) {
 #pragma unroll
             for (int c = 0; c < D; ++c) {
-                v[c] = p.v[c][j] + qmdt * e[c];
+                const T v0 = p.v[c][j];
+                v[c] = v0 + qmdt * e[c];
+                T xn = x[c] + dt * v[c];
+                if (!(xn >= (T)0 && xn < g.L[c])) xn = advance_wrap<T>(x[c], v0, e[c], dtd, qmdtd, g.Ld[c]);
                 p.v[c][j] = v[c];
-                p.x[c][j] = wrap_periodic(x[c] + dt * v[c], g.L[c], g.inv_L[c]);
+                p.x[c][j] = xn;
             }
         }
     }
@@ -178,11 +182,12 @@ __global__ void __launch_bounds__(128) k_strays(PartP<T> p, GridP<T> g, FieldP<T
 template <typename T, int D, int P, int MODE, bool VIA_PERM, int G_, bool STRAYS>
 __global__ void PIC_RUNS_BOUNDS(T)
 k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g, FieldP<T> f, int64_t n,
-       double* __restrict__ racc, T dt, T qmdt, const uint32_t* __restrict__ gate, uint32_t want,
+       double* __restrict__ racc, double dtd, double qmdtd, const uint32_t* __restrict__ gate, uint32_t want,
        uint32_t* __restrict__ stray_list, uint32_t* __restrict__ stray_count)
 {
     using SH = RunsShape<T, D, P, G_>;
     if (gate && *gate != want) return;                // the other arm of a device-side choice runs instead
+    const T dt = (T)dtd, qmdt = (T)qmdtd;
     constexpr int S = SH::S, S2 = S / 2, SZ = SH::SZ, ROWS = SH::ROWS;
     constexpr int G = SH::G, RPL = SH::RPL, NG = SH::NG, NV = SH::NV, NODES = SH::NODES, NPL = SH::NPL;
     constexpr int WR = SH::WR, RECS = SH::RECS;
@@ -514,21 +519,24 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
             const int64_t j = jl + b0;
             if (PUSH && !lonely) {
                 bool inside = true;
+                T e[D], vn[D], xn[D];
 #pragma unroll
                 for (int c = 0; c < D; ++c) {
                     T pe[G];
                     lds<T, G>(a_part + (uint32_t)((idx * D + c) * G) * B, pe);
-                    T e = pe[0];
+                    e[c] = pe[0];
 #pragma unroll
-                    for (int q = 1; q < G; ++q) e += pe[q];
-                    pv[c] += qmdt * e;
-                    px[c] += dt * pv[c];
-                    inside = inside && (px[c] >= (T)0 && px[c] < g.L[c]);
+                    for (int q = 1; q < G; ++q) e[c] += pe[q];
+                    vn[c] = pv[c] + qmdt * e[c];
+                    xn[c] = px[c] + dt * vn[c];
+                    inside = inside && (xn[c] >= (T)0 && xn[c] < g.L[c]);
                 }
                 if (!inside) {                        // one rare branch for all components
 #pragma unroll
-                    for (int c = 0; c < D; ++c) px[c] = wrap_periodic(px[c], g.L[c], g.inv_L[c]);
+                    for (int c = 0; c < D; ++c) xn[c] = advance_wrap<T>(px[c], pv[c], e[c], dtd, qmdtd, g.Ld[c]);
                 }
+#pragma unroll
+                for (int c = 0; c < D; ++c) { px[c] = xn[c]; pv[c] = vn[c]; }
             }
             if ((PUSH && !lonely) || VIA_PERM) {
 #pragma unroll
@@ -563,14 +571,14 @@ inline int launch_runs(const pic_grid_t& g, const pic_particles_t& src, const pi
     if (stray_list && stray_count) {
         auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, true>;
         kern<<<blocks, kRunsThreads, smem, st>>>(make_partp<T>(VIA_PERM ? src : dst), make_partp<T>(dst), perm,
-                                                make_gridp<T>(g), f, dst.n, racc, (T)dt, (T)(qm * dt), gate, want,
+                                                make_gridp<T>(g), f, dst.n, racc, dt, qm * dt, gate, want,
                                                 stray_list, stray_count);
         count_launch();
         return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
     }
     auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, false>;
     kern<<<blocks, kRunsThreads, smem, st>>>(make_partp<T>(VIA_PERM ? src : dst), make_partp<T>(dst), perm,
-                                            make_gridp<T>(g), f, dst.n, racc, (T)dt, (T)(qm * dt), gate, want,
+                                            make_gridp<T>(g), f, dst.n, racc, dt, qm * dt, gate, want,
                                             stray_list, stray_count);
     count_launch();
     return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
@@ -585,7 +593,7 @@ inline int launch_strays(const pic_grid_t& g, const pic_particles_t& p, const vo
     FieldP<T> f;
     for (int c = 0; c < 3; ++c) f.E[c] = (E && c < D) ? (const T*)E[c] : nullptr;
     k_strays<T, D, P, MODE><<<(unsigned)(sms * 8), 128, 0, st>>>(make_partp<T>(p), make_gridp<T>(g), f, stray_list, stray_count,
-                                                              racc, (T)dt, (T)(qm * dt));
+                                                              racc, dt, qm * dt);
     count_launch();
     return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
