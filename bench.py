@@ -60,13 +60,32 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r01_v5_final.md): key = "<config>:<phase of the dominant kernel>"
-NCU_TRAFFIC = {"cfg3:push": 8.38e9}          # 5.18 GB read + 3.20 GB written (profiles/r01_v5_final.md)
+def kernel_sources_sha256():
+    """Hash of the CUDA sources: ties a committed ncu traffic figure to the code it was captured on."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_1603_02886_b200", "csrc")
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()
 
 
 def ncu_traffic(cfg_name, kernel):
-    return NCU_TRAFFIC.get("%s:%s" % (cfg_name, kernel))
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+    `ncu --set full` capture listed in profiles/ncu_traffic.json -- only if that capture was taken on exactly
+    these kernel sources (sha256 recorded beside it); otherwise null, with the reason."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    try:
+        rec = json.load(open(p)).get("%s:%s" % (cfg_name, kernel))
+    except Exception:
+        rec = None
+    if not rec:
+        return None, "no ncu capture committed for this config and kernel"
+    if rec.get("sources_sha256") != kernel_sources_sha256():
+        return None, "stale: %s was captured on other kernel sources" % rec.get("source")
+    return float(rec["traffic_bytes"]), "%s (same kernel sources, sha256 %s)" % (rec.get("source"), rec["sources_sha256"][:12])
 
 
 class ClockSampler:
@@ -185,6 +204,7 @@ def main():
     ap.add_argument("--ppc", type=int, default=0, help="config 5: particles per cell")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cold", action="store_true")
     ap.add_argument("--ref-particles", type=int, default=2_000_000)
     ap.add_argument("--cpu-particles", type=int, default=30_000_000)
     args = ap.parse_args()
@@ -219,6 +239,16 @@ def main():
     cfg_rank = cfg.scaled(cfg.N, seed=cfg.seed + rank)          # replicas only: independent seeds
     g = B.grid_of(cfg_rank)
     wl = W.make_workload(cfg_rank)
+    # load every kernel of this configuration once on a scrap problem of the same shape, so that the first timed
+    # step below measures the step and not the lazy loading of the CUDA modules
+    tiny = cfg_rank.scaled(min(cfg_rank.N, 50_000))
+    wt = W.make_workload(tiny)
+    stt = B.Stepper(B.grid_of(tiny), wt.x, wt.v, wt.w, wt.E, device=dev)
+    for k in range(2):
+        stt.step(tiny.dt, tiny.qm, True)
+    stt.step(tiny.dt, tiny.qm, False)
+    torch.cuda.synchronize()
+    del stt, wt
     st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, device=dev)
     torch.cuda.synchronize()
 
@@ -294,8 +324,9 @@ def main():
         if B.FUSED_PHASE_IS_PUSH and dom == "push":
             bpp = B.fused_kernel_bytes(cfg.dim, 8 if cfg.dtype == "f64" else 4, sorts > 0)
         ach = bpp * cfg.N / (phase_ms[dom] * 1e-3) / 1e9
+        traffic, traffic_source = ncu_traffic(cfg.name, dom)
         roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
-                    "frac": ach / peak, "traffic": ncu_traffic(cfg.name, dom),
+                    "frac": ach / peak, "traffic": traffic, "traffic_source": traffic_source,
                     "peak_source": peak_src, "algorithmic_bytes_per_particle": bpp,
                     "kernel_ms": phase_ms[dom]}
     # second roof of the dominant kernel: plain fp32/fp64 arithmetic.  Algorithmic flops
@@ -313,6 +344,27 @@ def main():
                         "peak_source": "148 SMs x %d lanes x 2 flop x SM clock (DESIGN.md section 6)" % lanes}
     bytes_step = ab["step"] if cfg.sort_every == 1 else (ab["step"] * sorts + ab["nosort_step"] * (K - sorts)) / K
     step_ach = bytes_step * cfg.N / (ms_step * 1e-3) / 1e9
+
+    # ---- the configuration as BASELINE.json words it: its own number of steps FROM THE SEEDED, UNSORTED state
+    #      (the first step sorts every particle), one timed region, max over ranks
+    cold = None
+    if not args.no_cold:
+        nsteps = cfg.steps
+        st.reset(wl.x, wl.v, wl.w)
+        barrier()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record()
+        for k in range(nsteps):
+            st.step(cfg.dt, cfg.qm, do_sort=(k % cfg.sort_every == 0))
+        c1.record()
+        barrier()
+        cold_ms = max_over_ranks(c0.elapsed_time(c1), dist if world > 1 else None, dev)
+        cold_bytes = ab["step"] if cfg.sort_every == 1 else None
+        cold = {"steps": nsteps, "ms_total": cold_ms, "ms_per_step": cold_ms / nsteps,
+                "value": replica_throughput(cfg.N, world, nsteps, cold_ms), "unit": UNIT,
+                "what": "%d steps from the seeded random order (first step: every particle moves), as the config is stated" % nsteps}
+        if cold_bytes:
+            cold["frac_of_peak"] = cold_bytes * cfg.N / (cold_ms / nsteps * 1e-3) / 1e9 / peak
 
     # ---- end to end through the host-buffer entry point (pinned host memory, copies timed)
     e2e = None
@@ -346,7 +398,7 @@ def main():
             "cpu_baseline": cpu_baseline,
             "step_roofline": {"bytes_per_particle_step": bytes_step, "achieved": step_ach, "peak": peak,
                               "frac": step_ach / peak, "frac_of_8TBps_nominal": step_ach / 8000.0, "unit": "GB/s"},
-            "phase_ms": phase_ms, "first_step_ms": first_ms}
+            "phase_ms": phase_ms, "first_step_ms": first_ms, "cold": cold}
     if deposit_compare:
         line["deposit_ms"] = deposit_compare
     if e2e_resident:
@@ -450,7 +502,9 @@ def run_deposit_compare(B, torch, cfg, g, wl, st, dev, reps=5):
 
 
 def run_cpu_baseline(cfg, sample):
-    """The oracle as it stands (single thread) on a bounded sample of the same workload."""
+    """The oracle as it stands (single thread) on a bounded sample of the same workload, and the OpenMP build of
+    the same loops on every host core this process may use (the paper's CPU reference is OpenMP on 8 cores,
+    19.24 ns per particle and step)."""
     import oracle as O
     import pic_workloads as W
     sample = min(sample, cfg.N)
@@ -460,10 +514,22 @@ def run_cpu_baseline(cfg, sample):
     t0 = time.perf_counter()
     O.step(g, wl.x, wl.v, wl.w, wl.E, c.dt, c.qm)
     el = time.perf_counter() - t0
-    return {"value": sample / el, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": "first %d particles of %s on the full grid, 1 step (sort+deposit+push) from the seeded random order, %.1f s"
-                      % (sample, cfg.name, el),
-            "host_cores_available": os.cpu_count()}
+    what = "first %d particles of %s on the full grid, 1 step (sort+deposit+push) from the seeded random order" % (sample, cfg.name)
+    out = {"value": sample / el, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": "%s, %.1f s" % (what, el),
+           "host_cores_available": len(os.sched_getaffinity(0))}
+    try:
+        threads = len(os.sched_getaffinity(0))
+        O.build_openmp()
+        O.step_openmp(g, wl.x, wl.v, wl.w, wl.E, c.dt, c.qm, threads)          # thread pool start-up, page faults
+        t0 = time.perf_counter()
+        O.step_openmp(g, wl.x, wl.v, wl.w, wl.E, c.dt, c.qm, threads)
+        el2 = time.perf_counter() - t0
+        out["openmp"] = {"value": sample / el2, "unit": UNIT, "cores": threads, "kind": "oracle, OpenMP build of the same loops",
+                         "ns_per_particle_step": 1e9 * el2 / sample, "sample": "%s, %.1f s" % (what, el2),
+                         "paper_reference": "19.24 ns per particle and step, OpenMP, 8 cores of a Xeon E5-2670, linear splines, 2-D (PAPER.md:388)"}
+    except Exception as e:                                    # no OpenMP runtime on the box
+        out["openmp"] = {"unavailable": str(e)[:200]}
+    return out
 
 
 if __name__ == "__main__":

@@ -30,6 +30,40 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+_LIB_OMP = os.path.join(_HERE, "libpicref_omp.so")
+
+
+def build_openmp(force: bool = False) -> str:
+    """The TIMED-ONLY OpenMP build of the same source (bench.py's cpu_baseline; never used for parity)."""
+    if force or not os.path.exists(_LIB_OMP) or os.path.getmtime(_LIB_OMP) < os.path.getmtime(_SRC):
+        tmp = _LIB_OMP + ".%d.tmp" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+                               "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB_OMP)
+    return _LIB_OMP
+
+
+def step_openmp(g: "Grid", x, v, w, E, dt: float, qm: float, threads: int):
+    """pic_ref_step of the OpenMP build on `threads` host threads -> dict like step()."""
+    lib = ctypes.CDLL(build_openmp())
+    lib.pic_ref_step.restype = ctypes.c_int
+    omp = ctypes.CDLL("libgomp.so.1")
+    omp.omp_set_num_threads(int(threads))
+    n = w.shape[0]
+    xo = [np.empty_like(a) for a in x]
+    vo = [np.empty_like(a) for a in v]
+    wo = np.empty_like(w)
+    perm = np.empty(n, np.int32)
+    off = np.empty(g.cells + 1, np.int32)
+    rho = np.empty(g.cells, np.float64)
+    cg = g.c()
+    _rc(lib.pic_ref_step(ctypes.byref(cg), ctypes.c_int64(n), _ptrs(x), _ptrs(v), ctypes.c_void_p(w.ctypes.data),
+                         _ptrs(xo), _ptrs(vo), ctypes.c_void_p(wo.ctypes.data), ctypes.c_void_p(perm.ctypes.data),
+                         ctypes.c_void_p(off.ctypes.data), ctypes.c_void_p(rho.ctypes.data), _ptrs(E),
+                         ctypes.c_double(dt), ctypes.c_double(qm), ctypes.c_int(1)))
+    return dict(x=xo, v=vo, w=wo, perm=perm, cell_offsets=off, rho=rho)
+
+
 class _Grid(ctypes.Structure):
     _fields_ = [("dim", ctypes.c_int32), ("n", ctypes.c_int32 * 3), ("h", ctypes.c_double * 3),
                 ("order", ctypes.c_int32), ("dtype", ctypes.c_int32)]

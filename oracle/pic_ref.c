@@ -14,6 +14,14 @@
  * decided in the same precision on both sides.  Single thread, particle order,
  * stencil loops z-outer / y / x-inner.  No blocking, fusion or reordering.
  *
+ * A second, TIMED-ONLY build (oracle.build_openmp(): the same file with -fopenmp,
+ * libpicref_omp.so) spreads the particle loops of the key pass, the attribute move,
+ * the deposit (one private grid per thread, added up at the end) and the push over
+ * the host cores: it mirrors the paper's own CPU reference, OpenMP on 8 cores
+ * (PAPER.md:388), for bench.py's cpu_baseline.  Everything between `#ifdef _OPENMP`
+ * belongs to that build; the parity tests load the plain build only, whose
+ * arithmetic and order are as stated above.
+ *
  * Every function cites the passage of /root/reference/PAPER.md it follows
  * (PAPER.md:NNN = line NNN, with section).  Readings R1..R20 of silent or garbled
  * passages are listed in DESIGN.md.
@@ -200,10 +208,16 @@ int pic_ref_sort(const pic_ref_grid *g, int64_t n,
     if (!key || !cursor) { free(key); free(cursor); return REF_BAD_ARG; }
 
     for (int64_t k = 0; k <= C; ++k) cell_offsets[k] = 0;
+#ifdef _OPENMP                                           /* timed OpenMP build only, see the header */
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) key[i] = cell_key(g, xin, i);
+    for (int64_t i = 0; i < n; ++i) cell_offsets[key[i] + 1] += 1;
+#else
     for (int64_t i = 0; i < n; ++i) {                    /* histogram */
         key[i] = cell_key(g, xin, i);
         cell_offsets[key[i] + 1] += 1;
     }
+#endif
     for (int64_t k = 0; k < C; ++k)                      /* prefix sum */
         cell_offsets[k + 1] += cell_offsets[k];
     for (int64_t k = 0; k < C; ++k) cursor[k] = cell_offsets[k];
@@ -211,6 +225,9 @@ int pic_ref_sort(const pic_ref_grid *g, int64_t n,
         perm[cursor[key[i]]++] = (int32_t)i;
 
     size_t s = g->dtype ? 8 : 4;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
     for (int64_t j = 0; j < n; ++j) {                    /* move the attributes bit for bit */
         int64_t i = perm[j];
         for (int c = 0; c < g->dim; ++c) {
@@ -232,6 +249,24 @@ int pic_ref_sort(const pic_ref_grid *g, int64_t n,
  * normalisation are reading R2, chosen so that sum_j rho_j h^d = sum_i w_i.
  * rho is overwritten (reading R10).  Particle order; nodes z-outer/y/x-inner.
  * ------------------------------------------------------------------------- */
+static void deposit_one(const pic_ref_grid *g, const void *const x[3], const void *w, int64_t i,
+                        double inv_vol, double *rho)
+{
+    int32_t ix[3][4];
+    double wt[3][4];
+    int m[3] = {1, 1, 1};
+    ix[2][0] = 0; wt[2][0] = 1.0;
+    for (int c = 0; c < g->dim; ++c)
+        m[c] = stencil_1d(g, c, grid_coord(g, c, x[c], i), ix[c], wt[c]);
+    double q = load_real(g, w, i) * inv_vol;
+    for (int kz = 0; kz < m[2]; ++kz)
+        for (int ky = 0; ky < m[1]; ++ky)
+            for (int kx = 0; kx < m[0]; ++kx) {
+                int64_t j = ix[0][kx] + (int64_t)g->n[0] * (ix[1][ky] + (int64_t)g->n[1] * ix[2][kz]);
+                rho[j] += q * (wt[0][kx] * wt[1][ky] * wt[2][kz]);
+            }
+}
+
 int pic_ref_deposit(const pic_ref_grid *g, int64_t n, const void *const x[3], const void *w,
                     double *rho)
 {
@@ -241,21 +276,21 @@ int pic_ref_deposit(const pic_ref_grid *g, int64_t n, const void *const x[3], co
     for (int c = 0; c < g->dim; ++c) inv_vol /= g->h[c];
     for (int64_t k = 0; k < C; ++k) rho[k] = 0.0;
 
-    int32_t ix[3][4];
-    double wt[3][4];
-    for (int64_t i = 0; i < n; ++i) {
-        int m[3] = {1, 1, 1};
-        ix[2][0] = 0; wt[2][0] = 1.0;
-        for (int c = 0; c < g->dim; ++c)
-            m[c] = stencil_1d(g, c, grid_coord(g, c, x[c], i), ix[c], wt[c]);
-        double q = load_real(g, w, i) * inv_vol;
-        for (int kz = 0; kz < m[2]; ++kz)
-            for (int ky = 0; ky < m[1]; ++ky)
-                for (int kx = 0; kx < m[0]; ++kx) {
-                    int64_t j = ix[0][kx] + (int64_t)g->n[0] * (ix[1][ky] + (int64_t)g->n[1] * ix[2][kz]);
-                    rho[j] += q * (wt[0][kx] * wt[1][ky] * wt[2][kz]);
-                }
+#ifdef _OPENMP
+    /* Timed OpenMP build only (see the header): particles split over the threads, one private grid per
+     * thread, the grids added up at the end.  The summation order differs from the plain build. */
+#pragma omp parallel
+    {
+        double *priv = (double *)calloc((size_t)C, sizeof(double));
+#pragma omp for schedule(static)
+        for (int64_t i = 0; i < n; ++i) deposit_one(g, x, w, i, inv_vol, priv);
+#pragma omp critical
+        for (int64_t k = 0; k < C; ++k) rho[k] += priv[k];
+        free(priv);
     }
+#else
+    for (int64_t i = 0; i < n; ++i) deposit_one(g, x, w, i, inv_vol, rho);
+#endif
     return REF_OK;
 }
 
@@ -376,6 +411,9 @@ int pic_ref_push(const pic_ref_grid *g, int64_t n, void *const x[3], void *const
                  const void *const E[3], double dt, double qm)
 {
     if (!grid_ok(g) || n < 0) return REF_BAD_ARG;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
     for (int64_t i = 0; i < n; ++i) {
         double e[3];
         gather_one(g, (const void *const *)x, E, i, e);

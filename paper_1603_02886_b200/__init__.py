@@ -299,6 +299,16 @@ class Stepper:
         self.ws = torch.empty(pic_workspace_bytes(g, self.n), dtype=torch.uint8, device=dev)
         self.sorted_once = False
 
+    def reset(self, x, v, w):
+        """Start again from host arrays x, v, w (as if no step had been taken: no order hint)."""
+        import torch
+        for c in range(self.g.dim):
+            self.cur["x"][c].copy_(torch.as_tensor(x[c]))
+            self.cur["v"][c].copy_(torch.as_tensor(v[c]))
+        self.cur["w"].copy_(torch.as_tensor(w))
+        self.cell_offsets.zero_()
+        self.sorted_once = False
+
     def step(self, dt: float, qm: float, do_sort: bool = True, stream=None):
         a, b = self.cur, self.nxt
         if do_sort:
