@@ -22,6 +22,8 @@
  *  - Ownership: the caller owns every buffer, including the workspace; the library
  *    allocates nothing, frees nothing and keeps no particle or grid state between calls
  *    (the only per-thread state is the launch counter and the optional phase-event hook below).
+ *    What carries over from one call to the next lives in the caller's buffers: cell_offsets (an order
+ *    hint, see pic_sort) and, for PIC_SORT_CHAINED, the workspace (see pic_step).
  *  - Execution: all work is enqueued on `stream` (a cudaStream_t passed as void*);
  *    no host synchronisation and no host<->device copy happens inside ("data transfers
  *    ... kept to a minimum").  Results are valid once the stream is synced.
@@ -93,7 +95,13 @@ int pic_workspace_bytes(const pic_grid_t *grid, int64_t n, size_t *bytes /* host
  *       (PAPER.md:120-122); `out` must not alias `in` -- the caller ping-pongs instead of the
  *       paper's copy-back.
  * perm[N]          : int32, perm[j] = source index of the particle now at position j (R9).
- * cell_offsets[C+1]: int32, particles of cell k occupy [cell_offsets[k], cell_offsets[k+1]).
+ * cell_offsets[C+1]: int32, IN/OUT.  On return: particles of cell k occupy [cell_offsets[k], cell_offsets[k+1]).
+ *       On ENTRY the array is READ as an optional order hint: if it holds the offsets of an earlier sort of
+ *       these particles (in a time loop: the previous step's output) only the particles that have left their
+ *       interval since are sorted ("pre-ordered particles", Alg. 2).  The result
+ *       never depends on what the array holds -- any content, including uninitialised memory, gives the same
+ *       perm and offsets, only slower -- but the memory must be readable; zero it where a tool such as
+ *       compute-sanitizer initcheck is used.
  */
 int pic_sort(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t *out,
              int32_t *perm, int32_t *cell_offsets, void *ws, size_t ws_bytes, void *stream);
@@ -132,6 +140,17 @@ int pic_push(const pic_grid_t *grid, pic_particles_t *p, int order_state,
  * accel -> push, the paper's loop order setrho -> accel -> push with the
  * field solve left out as in the paper and the re-sort of PAPER.md:100 placed first (R6).
  * out receives the particles in sorted order, advanced to t+1; rho is the density at t.
+ * do_sort = PIC_SORT (1): sort by the keys of the positions in `in`; cell_offsets is read on entry as a hint and
+ *   overwritten, exactly as in pic_sort; `out` must not overlap `in`.
+ * do_sort = PIC_SORT_CHAINED (3): the same result, for a time loop.  The caller states that `in` is, UNMODIFIED,
+ *   the `out` of the previous pic_step(do_sort != 0) call made with this workspace.  That call's step kernel had
+ *   every advanced position in registers and left the next keys, their histogram and the list of particles that
+ *   changed cell in the workspace ("emission of next-step keys"), so this call's sort does not
+ *   read the positions again.  What can be checked is checked on the device (same N, grid and array addresses; the
+ *   workspace was not used by another sort or step in between): if it does not hold, the call behaves like
+ *   PIC_SORT.  What cannot be checked is the caller's statement itself: particle data changed in place between
+ *   the two calls gives a wrong order.  In a chain the hint is the workspace's own copy of the previous
+ *   offsets; cell_offsets is only written.
  * do_sort = 0: particles keep their order (out_a[j] = advanced in_a[j]; out may be the same arrays as
  * in); perm is not written and cell_offsets is not modified.  cell_offsets may be NULL (any-order
  * kernels) or the offsets of an EARLIER sort of these particles: they are then used to walk the
@@ -140,6 +159,8 @@ int pic_push(const pic_grid_t *grid, pic_particles_t *p, int order_state,
  * holds: offsets that cannot be walked (checked on the device: off[0] = 0, off[C] = N, non-decreasing)
  * select the any-order kernels.  This is config 5's "sort every 4 / 16 steps" arm.
  */
+#define PIC_SORT 1
+#define PIC_SORT_CHAINED 3
 int pic_step(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t *out,
              int32_t *perm, int32_t *cell_offsets, void *rho, const void *const E[3],
              double dt, double qm, int do_sort, void *ws, size_t ws_bytes, void *stream);

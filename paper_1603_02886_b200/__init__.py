@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libpic_b200.so")
 PIC_F32, PIC_F64 = 0, 1
 PIC_OK = 0
 PIC_ORDER_UNSORTED, PIC_ORDER_SORTED, PIC_ORDER_STALE = 0, 1, 2
+PIC_SORT, PIC_SORT_CHAINED = 1, 3
 
 EXPORTS = ("pic_workspace_bytes", "pic_sort", "pic_deposit", "pic_push", "pic_step",
            "pic_step_host_bytes", "pic_step_host", "pic_step_fields_host_bytes", "pic_step_fields_host",
@@ -237,8 +238,9 @@ def pic_push(g: Grid, x, v, E, dt: float, qm: float, order_state=PIC_ORDER_UNSOR
 
 
 def pic_step(g: Grid, x_in, v_in, w_in, x_out, v_out, w_out, perm, cell_offsets, rho, E, dt: float, qm: float,
-             do_sort: bool = True, ws=None, stream=None):
-    """sort (if do_sort) -> deposit at x(t) -> accel -> push.  out = particles in sorted order at t+1."""
+             do_sort=True, ws=None, stream=None):
+    """sort (if do_sort) -> deposit at x(t) -> accel -> push.  out = particles in sorted order at t+1.
+    do_sort: False / 0, True / PIC_SORT, or PIC_SORT_CHAINED (in = unmodified out of the previous step, see pic.h)."""
     n = w_in.numel()
     _dev_check(g, list(x_in) + list(v_in) + [w_in] + list(x_out) + list(v_out) + [w_out], n)
     _dev_check(g, list(E) + [rho], g.cells)
@@ -246,7 +248,7 @@ def pic_step(g: Grid, x_in, v_in, w_in, x_out, v_out, w_out, perm, cell_offsets,
     pi, po = _particles(g, x_in, v_in, w_in, n), _particles(g, x_out, v_out, w_out, n)
     wsb = ws.numel() * ws.element_size() if ws is not None else 0
     _check(lib().pic_step(ctypes.byref(cg), ctypes.byref(pi), ctypes.byref(po), _ptr(perm), _ptr(cell_offsets),
-                          _ptr(rho), _field(g, E), dt, qm, 1 if do_sort else 0, _ptr(ws), wsb, _stream(stream)),
+                          _ptr(rho), _field(g, E), dt, qm, int(do_sort), _ptr(ws), wsb, _stream(stream)),
            "pic_step")
 
 
@@ -298,6 +300,7 @@ class Stepper:
         self.rho = torch.empty(g.cells, dtype=g.torch_dtype, device=dev)
         self.ws = torch.empty(pic_workspace_bytes(g, self.n), dtype=torch.uint8, device=dev)
         self.sorted_once = False
+        self._chain_ok = False
 
     def reset(self, x, v, w):
         """Start again from host arrays x, v, w (as if no step had been taken: no order hint)."""
@@ -308,12 +311,18 @@ class Stepper:
         self.cur["w"].copy_(torch.as_tensor(w))
         self.cell_offsets.zero_()
         self.sorted_once = False
+        self._chain_ok = False       # the arrays were written from outside: the next sort reads the positions
 
-    def step(self, dt: float, qm: float, do_sort: bool = True, stream=None):
+    def step(self, dt: float, qm: float, do_sort: bool = True, stream=None, chained: bool = True):
+        """One pic_step on the resident particles.  chained: sort steps are PIC_SORT_CHAINED -- this object owns the
+        particle arrays and nothing else writes them between steps, which is what that flag states (the library
+        checks the rest, so the first step and a step after reset() or an unsorted step fall back by themselves)."""
         a, b = self.cur, self.nxt
         if do_sort:
             pic_step(self.g, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], self.perm, self.cell_offsets,
-                     self.rho, self.E, dt, qm, True, self.ws, stream)
+                     self.rho, self.E, dt, qm, PIC_SORT_CHAINED if (chained and self._chain_ok) else PIC_SORT,
+                     self.ws, stream)
+            self._chain_ok = True
             self.cur, self.nxt = b, a
             self.sorted_once = True
         else:   # in place, current order

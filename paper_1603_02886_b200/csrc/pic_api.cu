@@ -51,10 +51,13 @@ static int check_grid(const pic_grid_t* g)
     return PIC_OK;
 }
 
-static int check_particles(const pic_grid_t& g, const pic_particles_t* p, bool need_v, bool need_w)
+// n_override >= 0: p is an OUTPUT set whose own n is not read (it receives n_override particles)
+static int check_particles(const pic_grid_t& g, const pic_particles_t* p, bool need_v, bool need_w, int64_t n_override = -1)
 {
-    if (!p || p->n < 0 || p->n >= ((int64_t)1 << 30)) return PIC_ERR_INVALID_ARG;
-    if (p->n == 0) return PIC_OK;                      // empty arrays may be null
+    if (!p) return PIC_ERR_INVALID_ARG;
+    const int64_t n = n_override >= 0 ? n_override : p->n;
+    if (n < 0 || n >= ((int64_t)1 << 30)) return PIC_ERR_INVALID_ARG;
+    if (n == 0) return PIC_OK;                         // empty arrays may be null
     for (int c = 0; c < g.dim; ++c) {
         if (!aligned16(p->x[c])) return PIC_ERR_INVALID_ARG;
         if (need_v && !aligned16(p->v[c])) return PIC_ERR_INVALID_ARG;
@@ -63,16 +66,21 @@ static int check_particles(const pic_grid_t& g, const pic_particles_t* p, bool n
     return PIC_OK;
 }
 
-static bool aliases(const pic_grid_t& g, const pic_particles_t& a, const pic_particles_t& b)
+// does any array of a overlap any array of b (n elements each)?
+static bool aliases(const pic_grid_t& g, const pic_particles_t& a, const pic_particles_t& b, int64_t n)
 {
-    const void* pa[7];
-    const void* pb[7];
+    const char* pa[7];
+    const char* pb[7];
     int m = 0;
-    for (int c = 0; c < g.dim; ++c) { pa[m] = a.x[c]; pb[m++] = b.x[c]; pa[m] = a.v[c]; pb[m++] = b.v[c]; }
-    pa[m] = a.w; pb[m++] = b.w;
+    for (int c = 0; c < g.dim; ++c) {
+        pa[m] = (const char*)a.x[c]; pb[m++] = (const char*)b.x[c];
+        pa[m] = (const char*)a.v[c]; pb[m++] = (const char*)b.v[c];
+    }
+    pa[m] = (const char*)a.w; pb[m++] = (const char*)b.w;
+    const size_t bytes = (size_t)n * (g.dtype == PIC_F64 ? 8 : 4);
     for (int i = 0; i < m; ++i)
         for (int j = 0; j < m; ++j)
-            if (pa[i] == pb[j]) return true;
+            if (pa[i] < pb[j] + bytes && pb[j] < pa[i] + bytes) return true;
     return false;
 }
 
@@ -128,14 +136,14 @@ int pic_sort(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
     int rc = check_grid(grid);
     if (rc != PIC_OK) return rc;
     if ((rc = check_particles(*grid, in, true, true)) != PIC_OK) return rc;
-    if ((rc = check_particles(*grid, out, true, true)) != PIC_OK) return rc;
+    if ((rc = check_particles(*grid, out, true, true, in->n)) != PIC_OK) return rc;
     if ((in->n > 0 && !aligned16(perm)) || !aligned16(cell_offsets) || !aligned16(ws)) return PIC_ERR_INVALID_ARG;
-    if (in->n > 0 && aliases(*grid, *in, *out)) return PIC_ERR_INVALID_ARG;
+    if (in->n > 0 && aliases(*grid, *in, *out, in->n)) return PIC_ERR_INVALID_ARG;
     SortWs sws;
     if ((rc = carve_sort_ws(*grid, in->n, ws, ws_bytes, sws)) != PIC_OK) return rc;
     pic_particles_t o = *out;
     o.n = in->n;
-    return launch_sort(*grid, *in, o, perm, cell_offsets, sws, true, (cudaStream_t)stream);
+    return launch_sort(*grid, *in, o, perm, cell_offsets, sws, true, false, (cudaStream_t)stream);
 }
 
 int pic_deposit(const pic_grid_t* grid, const pic_particles_t* p, int order_state, const int32_t* cell_offsets,
@@ -184,8 +192,9 @@ int pic_step(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
     g_launches = 0;
     int rc = check_grid(grid);
     if (rc != PIC_OK) return rc;
+    if (do_sort != 0 && do_sort != PIC_SORT && do_sort != PIC_SORT_CHAINED) return PIC_ERR_INVALID_ARG;
     if ((rc = check_particles(*grid, in, true, true)) != PIC_OK) return rc;
-    if ((rc = check_particles(*grid, out, true, true)) != PIC_OK) return rc;
+    if ((rc = check_particles(*grid, out, true, true, in->n)) != PIC_OK) return rc;
     if ((rc = check_field(*grid, E)) != PIC_OK) return rc;
     if (!aligned16(rho)) return PIC_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
@@ -197,9 +206,9 @@ int pic_step(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
     if ((rc = carve_sort_ws(*grid, in->n, ws, ws_bytes, sws)) != PIC_OK) return rc;
     if (do_sort) {
         if ((in->n > 0 && !aligned16(perm)) || !aligned16(cell_offsets)) return PIC_ERR_INVALID_ARG;
-        if (in->n > 0 && aliases(*grid, *in, *out)) return PIC_ERR_INVALID_ARG;
+        if (in->n > 0 && aliases(*grid, *in, *out, in->n)) return PIC_ERR_INVALID_ARG;
         // perm and cell_offsets only: the reorder itself happens inside the fused kernel below
-        if ((rc = launch_sort(*grid, *in, o, perm, cell_offsets, sws, false, st)) != PIC_OK) return rc;
+        if ((rc = launch_sort(*grid, *in, o, perm, cell_offsets, sws, false, (do_sort & PIC_SORT_CHAINED) == PIC_SORT_CHAINED, st)) != PIC_OK) return rc;
     } else {
         // keep the current order; out may be the same arrays as in (in-place step)
         for (int c = 0; c < grid->dim; ++c) {
@@ -222,6 +231,7 @@ int pic_step(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
         mark_phase(PIC_PHASE_PUSH, st);
         return rc;
     }
+    PIC_CUDA_OK(cudaMemsetAsync(sws.chain_sig, 0, sizeof(ChainSig), st));       // positions change: no chain from here
     if ((rc = launch_deposit(*grid, o, PIC_ORDER_UNSORTED, nullptr, rho, sws.racc, st)) != PIC_OK) return rc;
     mark_phase(PIC_PHASE_DEPOSIT, st);
     rc = launch_push(*grid, o, PIC_ORDER_UNSORTED, nullptr, E, dt, qm, st);
@@ -308,7 +318,8 @@ int pic_step_host(const pic_grid_t* grid, const pic_particles_t* in, pic_particl
     if (!do_sort && cell_offsets)
         PIC_CUDA_OK(cudaMemcpyAsync(doff, cell_offsets, 4 * (C + 1), cudaMemcpyHostToDevice, st));
 
-    rc = pic_step(grid, &din, &dout, dperm, (do_sort || cell_offsets) ? doff : nullptr, drho, dE, dt, qm, do_sort,
+    rc = pic_step(grid, &din, &dout, dperm, (do_sort || cell_offsets) ? doff : nullptr, drho, dE, dt, qm,
+                  do_sort ? PIC_SORT : 0,              // the particles arrive afresh with every call: never a chain
                   b + L.ws, L.ws_bytes, stream);
     if (rc != PIC_OK) return rc;
     const int launches = g_launches;

@@ -166,6 +166,35 @@ void count_launch(int n = 1);
 // records the caller's event for `phase` on `st` if pic_set_phase_events() installed one
 void mark_phase(int phase, cudaStream_t st);
 
+// positions per staging tile of the movers (k_classify: half a block; k_runs: one warp's range)
+constexpr int kStageTile = 2048;
+
+// What a step kernel leaves behind for the NEXT step's sort (row a8: "emission of next-step keys + histogram").
+// The advanced position of slot j is in registers, so its next cell key costs a few instructions here instead of a
+// pass over x[d] there.  Slot j lies in the interval of its present key in this step's cell_offsets -- which are the
+// next sort's hint -- so "stays in its interval" is simply new key == present key, and "comes from below the
+// interval of its new key" is new key > present key (the intervals are ordered by key): no offsets are read.
+// The layout is k_classify's (pic_sort.cu): tiles of kStageTile positions = one warp's range here.
+struct EmitP {
+    uint32_t* pkey;          // [N] next key of every slot
+    uint32_t* mask;          // [N/32] mover bits of every 32 slots
+    uint32_t* mprefix;       // [N/32] movers before the word, within its tile
+    uint32_t* stage_key;     // [N] movers of tile t, in slot order, from t*kStageTile on: next key ...
+    uint32_t* stage_idx;     //     ... and slot
+    int32_t* tile_count;     // [tiles] movers of the tile
+    int32_t* cell_out;       // [C] particles that leave cell k                        (zeroed by the caller)
+    unsigned long long* mover_in;   // [C] low word: movers into cell k; high word: those of them that come from below
+};
+
+// What identifies the particle set a chain of pic_step calls works on (see PIC_SORT_CHAINED in pic.h): written
+// to the workspace after a step, compared with the next call's arguments on the device.
+struct ChainSig {
+    uint64_t magic;          // kChainMagic when a step has left its emission behind, else anything
+    uint64_t n, cells, grid; // particles, cells, hash of the grid parameters
+    uint64_t arr[7];         // the arrays that hold the particles (out of the step that wrote it = in of the next)
+};
+constexpr uint64_t kChainMagic = 0x50494332434841ull;     // "PIC2CHA"
+
 // ---- launchers implemented in the .cu files (all enqueue on `st`) ------------------------
 struct SortWs {
     uint32_t* keys[2];       // [N] movers' keys, ping-pong
@@ -179,29 +208,39 @@ struct SortWs {
     int32_t* tile_count;     // [classify tiles] movers per tile
     int32_t* tile_base;      // [classify tiles + 1] exclusive scan of tile_count
     uint32_t* lookback;      // [passes][radix tiles][kRadix]
-    int32_t* cell_count;     // [C+1] histogram of the keys              (zero region from here ...)
+    int32_t* cell_count;     // [C+1] histogram of the keys              (hist region: these three)
     int32_t* mover_count;    // [C+1] histogram of the movers' keys
     int32_t* mover_lo;       // [C+1] movers into a cell from below its hint interval
-    uint32_t* digit_hist;    // [kMaxPasses][kRadix]
+    uint32_t* digit_hist;    // [kMaxPasses][kRadix]                      (zero region from here ...)
     uint32_t* scan_status;   // [2][scan tiles]
     uint32_t* cls_status;    // [scan tiles of the classify tiles]
-    uint32_t* counters;      // [64] tile tickets, number of movers, hint flag  (... to here)
+    uint32_t* counters;      // [64] tile tickets, number of movers, hint and chain flags  (... to here)
     uint32_t* gate;          // one word of counters: 1 = more than half of the particles are movers (set by the sort)
     uint32_t* stray_count;   // one word of counters: particles the step kernel has set aside (zeroed with the counters)
     uint32_t* stray_list;    // [N] their slots (= idx[0]: free once perm is written)
     double* racc;            // [C] double accumulation grid of the deposit (not in the zero region)
+    int32_t* prev_off;       // [C+1] cell_offsets as the last sort of a chain wrote them (the next one's hint)
+    ChainSig* chain_sig;     // what that step worked on
+    EmitP emit;              // where a step kernel leaves the next sort's inputs
+    void* hist_begin;        // cell_count, mover_count, mover_lo: zeroed before k_classify, written by k_chain_counts in a chain
+    size_t hist_bytes;
+    void* emit_begin;        // emit.cell_out, emit.mover_in: zeroed before an emitting step kernel
+    size_t emit_bytes;
     void* zero_begin;        // region that must be zero before a sort
     size_t zero_bytes;
     int passes, bits_per_pass, key_bits;
-    int64_t radix_tiles, scan_tiles, cls_tiles;
+    int64_t radix_tiles, scan_tiles, cls_tiles, stage_tiles;
 };
 
 size_t sort_ws_bytes(const pic_grid_t& g, int64_t n);
 int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, SortWs& out);
 
-// reorder = false: only perm and cell_offsets are produced (out is not written)
+// reorder = false: only perm and cell_offsets are produced (out is not written).  chained: the caller says that
+// `in` is the unmodified output of the previous pic_step on this workspace (checked on the device against the
+// workspace's ChainSig): keys, histograms and the stayer/mover split are then the ones that step emitted.
 int launch_sort(const pic_grid_t& g, const pic_particles_t& in, pic_particles_t& out, int32_t* perm,
-                int32_t* cell_offsets, const SortWs& ws, bool reorder, cudaStream_t st);
+                int32_t* cell_offsets, const SortWs& ws, bool reorder, bool chained, cudaStream_t st);
+int launch_chain_commit(const pic_grid_t& g, const pic_particles_t& out, const SortWs& ws, cudaStream_t st);
 int launch_deposit(const pic_grid_t& g, const pic_particles_t& p, int order_state,
                    const int32_t* cell_offsets, void* rho, double* racc, cudaStream_t st);
 int launch_push(const pic_grid_t& g, pic_particles_t& p, int order_state, const int32_t* cell_offsets,

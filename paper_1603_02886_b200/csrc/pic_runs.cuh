@@ -179,12 +179,15 @@ __global__ void __launch_bounds__(128) k_strays(PartP<T> p, GridP<T> g, FieldP<T
 }
 
 // STRAYS: lone particles are set aside in stray_list for k_strays (used where the order may be stale)
-template <typename T, int D, int P, int MODE, bool VIA_PERM, int G_, bool STRAYS>
+// EMIT:   the next sort's inputs are written as the particles are pushed (sorted input only: !STRAYS)
+template <typename T, int D, int P, int MODE, bool VIA_PERM, int G_, bool STRAYS, bool EMIT>
 __global__ void PIC_RUNS_BOUNDS(T)
 k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g, FieldP<T> f, int64_t n,
        double* __restrict__ racc, double dtd, double qmdtd, const uint32_t* __restrict__ gate, uint32_t want,
-       uint32_t* __restrict__ stray_list, uint32_t* __restrict__ stray_count)
+       uint32_t* __restrict__ stray_list, uint32_t* __restrict__ stray_count, EmitP em)
 {
+    static_assert(!EMIT || (!STRAYS && (MODE & kModePush) != 0), "emission needs the push and exact cell order");
+    static_assert(!EMIT || PIC_RUNS_WR == kStageTile, "one warp's range is one staging tile");
     using SH = RunsShape<T, D, P, G_>;
     if (gate && *gate != want) return;                // the other arm of a device-side choice runs instead
     const T dt = (T)dtd, qmdt = (T)qmdtd;
@@ -216,11 +219,11 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
     int cur = -1, ccx = 0, ccy = 0, ccz = 0;
     int since = 0;                                    // particles added to the node sums since the last full flush
     Pk<T> Er[PUSH ? D : 1][RPL][S2];                  // field on (row, slot pair)
-    T acc[DEP ? RPL : 1][S];                          // rho sums on (row, slot); scalars: ptxas copies loop-carried pairs
+    Pk<T> acc[DEP ? RPL : 1][S2];                     // rho sums on (row, slot pair)
 #pragma unroll
     for (int rr = 0; rr < (DEP ? RPL : 1); ++rr)
 #pragma unroll
-        for (int i = 0; i < S; ++i) acc[rr][i] = (T)0;
+        for (int i = 0; i < S2; ++i) acc[rr][i] = pk_zero<T>();
     int nidx[NPL];                                    // grid index of stencil position lane + 32 m = row*S + slot
     int rowb = 0;                                     // grid index of (x = 0, row lane mod ROWS)
 #pragma unroll
@@ -231,9 +234,10 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
         const uint32_t mine = a_buf + (uint32_t)(grp * NODES + lg * NV) * B;
 #pragma unroll
         for (int rr = 0; rr < RPL; ++rr) {
-            sts<T, S>(mine + rr * S * B, acc[rr]);
+            T a[S];
 #pragma unroll
-            for (int i = 0; i < S; ++i) acc[rr][i] = (T)0;
+            for (int i = 0; i < S2; ++i) { a[2 * i] = pk_lo(acc[rr][i]); a[2 * i + 1] = pk_hi(acc[rr][i]); acc[rr][i] = pk_zero<T>(); }
+            sts<T, S>(mine + rr * S * B, a);
         }
         __syncwarp();
 #pragma unroll
@@ -312,7 +316,11 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
             for (int s = 0; s < S; ++s)
                 if (rho == s) {                       // warp-uniform
 #pragma unroll
-                    for (int rr = 0; rr < RPL; ++rr) { col[rr] = acc[rr][s]; acc[rr][s] = (T)0; }
+                    for (int rr = 0; rr < RPL; ++rr) {
+                        const Pk<T> a = acc[rr][s / 2];
+                        col[rr] = (s & 1) ? pk_hi(a) : pk_lo(a);
+                        acc[rr][s / 2] = (s & 1) ? pk_make(pk_lo(a), (T)0) : pk_make((T)0, pk_hi(a));
+                    }
                 }
             sts<T, RPL>(a_buf + (uint32_t)(grp * ROWS + lg * RPL) * B, col);
             __syncwarp();
@@ -361,6 +369,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
 #pragma unroll
     for (int c = 0; c < D; ++c) { nx[c] = (T)0; nv[c] = (T)0; }
     int in1 = 0;                                      // source index of this lane's slot in batch b+1 (then b+2)
+    uint32_t emitted = 0;                             // EMIT: movers of this warp's range so far
     auto load_attrs = [&](int i) {
 #pragma unroll
         for (int c = 0; c < D; ++c) {
@@ -481,6 +490,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
 #pragma unroll
                 for (int i = 0; i < S2; ++i) wx2[i] = pk_make(wxv[2 * i], wxv[2 * i + 1]);
                 Pk<T> sum[PUSH ? D : 1];
+                const Pk<T> q2 = pk_make(qv, qv);
                 bool first = true;
 #pragma unroll
                 for (int rr = 0; rr < RPL; ++rr) {
@@ -489,10 +499,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
 #pragma unroll
                     for (int i = 0; i < S2; ++i) {
                         const Pk<T> pp = pk_mul(a2, wx2[i]);
-                        if constexpr (DEP) {
-                            acc[rr][2 * i] = fma(qv, pk_lo(pp), acc[rr][2 * i]);
-                            acc[rr][2 * i + 1] = fma(qv, pk_hi(pp), acc[rr][2 * i + 1]);
-                        }
+                        if constexpr (DEP) pk_acc(acc[rr][i], q2, pp);
                         if constexpr (PUSH) {
 #pragma unroll
                             for (int c = 0; c < D; ++c) {
@@ -544,6 +551,35 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
                 if constexpr (VIA_PERM) dst.w[j] = pw;
             }
         }
+        if constexpr (EMIT) {
+            // next key of the advanced particle: the same function of the stored position that k_classify applies
+            int nk = 0, mul = 1;
+#pragma unroll
+            for (int c = 0; c < D; ++c) {
+                nk += mul * cell_index(grid_coord(px[c], g.h[c], g.inv_h[c], g.hmul), g.n[c]);
+                mul *= g.n[c];
+            }
+            const bool mover = valid && nk != key;
+            const unsigned bal = __ballot_sync(FULL, mover);
+            if (valid) em.pkey[jl + b0] = (uint32_t)nk;
+            if (mover) {
+                const uint32_t at = (uint32_t)j0 + emitted + (uint32_t)__popc(bal & ((1u << lane) - 1u));
+                em.stage_key[at] = (uint32_t)nk;
+                em.stage_idx[at] = (uint32_t)(jl + b0);
+                // histograms: one particle fewer in the present cell, one mover more in the next one (the second
+                // word counts those that come from below); the sort puts count = old count - out + in together
+                atomicAdd(&em.cell_out[key], 1);
+                atomicAdd(&em.mover_in[nk], (nk > key) ? 0x100000001ull : 1ull);
+            }
+            if (lane == 0) {
+                em.mask[(j0 + b0) >> 5] = bal;
+                em.mprefix[(j0 + b0) >> 5] = emitted;
+            }
+            emitted += (uint32_t)__popc(bal);
+        }
+    }
+    if constexpr (EMIT) {
+        if (lane == 0) em.tile_count[j0 / WR] = (int32_t)emitted;
     }
     if (DEP && since > 0) flush_all();
     if constexpr (PUSH) cp_async_wait();              // a column fetched ahead may still be in flight
@@ -552,12 +588,13 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
 // launch k_runs over n particles.  VIA_PERM: particle perm[j] of src -> slot j of dst; otherwise in place
 // on dst.  racc = double accumulation grid of the deposit.  The kernel runs only if *gate == want (gate
 // may be NULL).  stray_list / stray_count (both or neither; *stray_count zeroed by the caller): lone particles
-// are set aside there for launch_strays instead of breaking the run they sit in.
+// are set aside there for launch_strays instead of breaking the run they sit in.  emit != NULL (MODE both, no
+// strays): the next sort's inputs are written too.
 template <typename T, int D, int P, int MODE, bool VIA_PERM>
 inline int launch_runs(const pic_grid_t& g, const pic_particles_t& src, const pic_particles_t& dst,
                        const int32_t* perm, const void* const E[3], double* racc, double dt, double qm,
                        cudaStream_t st, const uint32_t* gate = nullptr, uint32_t want = 0,
-                       uint32_t* stray_list = nullptr, uint32_t* stray_count = nullptr)
+                       uint32_t* stray_list = nullptr, uint32_t* stray_count = nullptr, const EmitP* emit = nullptr)
 {
     if (dst.n <= 0) return PIC_OK;
     constexpr int GP = sizeof(T) == 4 ? PIC_RUNS_G32 : PIC_RUNS_G64;
@@ -568,18 +605,29 @@ inline int launch_runs(const pic_grid_t& g, const pic_particles_t& src, const pi
     static_assert(smem <= 48 * 1024, "k_runs relies on the default dynamic shared memory limit");
     constexpr int64_t per_block = (int64_t)SH::WR * kRunsWarps;
     const unsigned blocks = (unsigned)((dst.n + per_block - 1) / per_block);
+    const EmitP none{};
+    if constexpr (MODE == kModeBoth) {
+        if (emit) {
+            auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, false, true>;
+            kern<<<blocks, kRunsThreads, smem, st>>>(make_partp<T>(VIA_PERM ? src : dst), make_partp<T>(dst), perm,
+                                                    make_gridp<T>(g), f, dst.n, racc, dt, qm * dt, gate, want,
+                                                    nullptr, nullptr, *emit);
+            count_launch();
+            return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+        }
+    }
     if (stray_list && stray_count) {
-        auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, true>;
+        auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, true, false>;
         kern<<<blocks, kRunsThreads, smem, st>>>(make_partp<T>(VIA_PERM ? src : dst), make_partp<T>(dst), perm,
                                                 make_gridp<T>(g), f, dst.n, racc, dt, qm * dt, gate, want,
-                                                stray_list, stray_count);
+                                                stray_list, stray_count, none);
         count_launch();
         return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
     }
-    auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, false>;
+    auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, false, false>;
     kern<<<blocks, kRunsThreads, smem, st>>>(make_partp<T>(VIA_PERM ? src : dst), make_partp<T>(dst), perm,
                                             make_gridp<T>(g), f, dst.n, racc, dt, qm * dt, gate, want,
-                                            stray_list, stray_count);
+                                            stray_list, stray_count, none);
     count_launch();
     return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }

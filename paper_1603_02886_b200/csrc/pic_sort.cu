@@ -30,6 +30,7 @@
 //           k_perm_movers / k_perm_stayers   perm
 //           k_reorder        out_a[j] = in_a[perm[j]] for every attribute (pic_sort only)
 #include <cmath>
+#include <cstring>
 
 #include "pic_common.cuh"
 
@@ -61,7 +62,7 @@ constexpr int kClsWarps = kClsThreads / 32;
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagPrefix = 2u << 30, kValMask = (1u << 30) - 1;
 
 // slots of SortWs::counters
-enum { kCtrScanA = 0, kCtrScanB = 1, kCtrCls = 2, kCtrRadix = 3 /* .. +kMaxPasses */, kCtrMovers = 8, kCtrHintBad = 9, kCtrGate = 16, kCtrStrays = 17 };
+enum { kCtrScanA = 0, kCtrScanB = 1, kCtrCls = 2, kCtrRadix = 3 /* .. +kMaxPasses */, kCtrMovers = 8, kCtrHintBad = 9, kCtrGate = 16, kCtrStrays = 17, kCtrChain = 18 };
 
 __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p)
 {
@@ -98,18 +99,66 @@ __device__ __forceinline__ uint32_t warp_lookback(uint32_t* status, int tile, ui
 }
 
 // ----------------------------------------------------------------------------- the hint
-// private copy of cell_offsets as found on entry; bad = 1 unless 0 <= h[0] <= h[1] <= ... <= h[C] <= N
-__global__ void __launch_bounds__(256) k_hint_check(const int32_t* __restrict__ hint, int32_t* __restrict__ old_off, int C,
-                                                    int64_t n, uint32_t* counters)
+// Is this call the next link of a chain (PIC_SORT_CHAINED, pic.h)?  Only if the caller asks for it AND the
+// workspace holds the emission of a step that wrote exactly the arrays this call reads.
+__device__ __forceinline__ bool chain_holds(const ChainSig* sig, const ChainSig& want)
 {
+    bool ok = sig->magic == kChainMagic && sig->n == want.n && sig->cells == want.cells && sig->grid == want.grid;
+#pragma unroll
+    for (int a = 0; a < 7; ++a) ok = ok && sig->arr[a] == want.arr[a];
+    return ok;
+}
+
+// private copy of the hint: cell_offsets as found on entry, or -- in a chain -- the offsets the previous step
+// wrote (kept in the workspace, so that the emitted stayer/mover split and the hint cannot disagree);
+// bad = 1 unless 0 <= h[0] <= h[1] <= ... <= h[C] <= N
+__global__ void __launch_bounds__(256) k_hint_check(const int32_t* __restrict__ hint, const int32_t* __restrict__ prev_off,
+                                                    const ChainSig* __restrict__ sig, ChainSig want, int chain_req,
+                                                    int32_t* __restrict__ old_off, int C, int64_t n, uint32_t* counters)
+{
+    __shared__ int s_chain;
+    if (threadIdx.x == 0) {
+        s_chain = (chain_req && chain_holds(sig, want)) ? 1 : 0;
+        if (blockIdx.x == 0) counters[kCtrChain] = (uint32_t)s_chain;
+    }
+    __syncthreads();
+    const int32_t* __restrict__ h = s_chain ? prev_off : hint;
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k > C) return;
-    const int32_t a = hint[k];
+    const int32_t a = h[k];
     old_off[k] = a;
     bool bad = a < 0 || (int64_t)a > n;
-    if (k < C) bad = bad || hint[k + 1] < a;
+    if (k < C) bad = bad || h[k + 1] < a;
     if (bad) counters[kCtrHintBad] = 1u;
 }
+
+// the three histograms are zero before k_classify fills them; in a chain the previous step kernel has filled them
+__global__ void __launch_bounds__(256) k_zero_hist(uint4* __restrict__ p, size_t n16, const uint32_t* __restrict__ counters)
+{
+    if (counters[kCtrChain]) return;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x)
+        p[i] = make_uint4(0u, 0u, 0u, 0u);
+}
+
+// In a chain the three histograms come from what the previous step kernel counted: particles that left each cell,
+// movers into it, and how many of those come from below.  count = old count - out + in.
+__global__ void __launch_bounds__(256) k_chain_counts(const int32_t* __restrict__ old_off, const int32_t* __restrict__ cell_out,
+                                                      const unsigned long long* __restrict__ mover_in, int32_t* __restrict__ cell_count,
+                                                      int32_t* __restrict__ mover_count, int32_t* __restrict__ mover_lo, int C,
+                                                      const uint32_t* __restrict__ counters)
+{
+    if (!counters[kCtrChain]) return;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= C) return;
+    const unsigned long long in = mover_in[k];
+    const int32_t min = (int32_t)(uint32_t)in;
+    mover_count[k] = min;
+    mover_lo[k] = (int32_t)(uint32_t)(in >> 32);
+    cell_count[k] = old_off[k + 1] - old_off[k] - cell_out[k] + min;
+}
+
+// the step has left its emission behind: the next call may chain on to it
+__global__ void k_chain_commit(ChainSig* sig, ChainSig now) { *sig = now; }
 
 // ----------------------------------------------------------------------------- keys, histograms, stayer/mover split
 // a1: key = c_x + n_x*(c_y + n_y*c_z) (x fastest), clamped cell index
@@ -145,6 +194,7 @@ struct BlockHist {
     }
 };
 static_assert(kClsTile <= (1 << 12), "13-bit fields of BlockHist");
+static_assert(kClsTile % kStageTile == 0 && kStageTile % (32 * kClsIPT) == 0, "staging tiles are whole warps of a classify block");
 
 // One warp's 32*kClsIPT positions.  CHECK = false: all of them are below n (no bounds tests).
 template <typename T, int D, bool CHECK>
@@ -243,6 +293,7 @@ k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, i
            int32_t* __restrict__ tile_count, uint32_t* __restrict__ pkey, const uint32_t* __restrict__ counters)
 {
     __shared__ uint32_t s_wsum[kClsWarps];
+    if (counters[kCtrChain]) return;                  // a chain: the previous step kernel has done this work
     const unsigned tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = (int)blockIdx.x;
     const bool hint_ok = counters[kCtrHintBad] == 0u;
@@ -266,14 +317,21 @@ k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, i
     for (int r = 0; r < kClsIPT; ++r) { wpre[r] = wtotal; wtotal += __popc(bal[r]); }
     if (lane == 0) s_wsum[warp] = wtotal;
     __syncthreads();
+    // movers are staged per kStageTile positions (one warp's range in the step kernel, which writes the same
+    // layout when it emits): this block covers kClsTile / kStageTile of them
+    constexpr int kWarpsPerStage = kStageTile / (32 * kClsIPT);
+    const int half = (int)warp / kWarpsPerStage;
     uint32_t warp_off = 0, total = 0;
 #pragma unroll
     for (int w = 0; w < kClsWarps; ++w) {
         const uint32_t t = s_wsum[w];
-        if (w < (int)warp) warp_off += t;
-        total += t;
+        if (w / kWarpsPerStage == half) {
+            if (w < (int)warp) warp_off += t;
+            total += t;
+        }
     }
-    if (tid == 0) tile_count[tile] = (int32_t)total;
+    if ((int)tid % (32 * kWarpsPerStage) == 0 && (int64_t)(tile * (kClsTile / kStageTile) + half) * kStageTile < n)
+        tile_count[tile * (kClsTile / kStageTile) + half] = (int32_t)total;
     // the block's histograms go to the grid arrays: one atomic per key and histogram (after the barrier above)
     for (int q = tid; q < kHashSize; q += kClsThreads) {
         const uint32_t k = s_hkey[q];
@@ -286,7 +344,7 @@ k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, i
     }
     // tile-relative for now: k_movers_place adds the movers of the tiles before this one
     const uint32_t base = warp_off;
-    const int stage = tile * kClsTile;
+    const int stage = tile * kClsTile + half * kStageTile;
     const unsigned lt = (1u << lane) - 1;
     // lane r writes the mask and prefix words of row r (the ballots are the same in every lane)
     {
@@ -310,30 +368,31 @@ k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, i
     }
 }
 
-// The movers of tile t, staged by k_classify at [t*kClsTile, ...), move to their place in the global
-// list: tile_base[t] = number of movers in the tiles before t (exclusive scan of tile_count).  The
-// per-word mover prefixes become global too.
-__global__ void __launch_bounds__(kClsThreads)
+// The movers of staging tile t (written by k_classify, or by the previous step kernel in a chain) move from
+// [t*kStageTile, ...) to their place in the global list: tile_base[t] = number of movers in the tiles before t
+// (exclusive scan of tile_count).  The per-word mover prefixes become global too.
+__global__ void __launch_bounds__(256)
 k_movers_place(const uint32_t* __restrict__ stage_key, const uint32_t* __restrict__ stage_idx, uint32_t* __restrict__ mkey,
                uint32_t* __restrict__ midx, uint32_t* __restrict__ mask, uint32_t* __restrict__ mprefix,
-               const int32_t* __restrict__ tile_base, int ntiles, int64_t n, uint32_t* counters)
+               const int32_t* __restrict__ tile_base, int ntiles, int64_t n, uint32_t* counters, ChainSig* sig)
 {
     const int tile = (int)blockIdx.x, tid = threadIdx.x;
     const uint32_t base = (uint32_t)tile_base[tile];
     const int cnt = tile_base[tile + 1] - tile_base[tile];
-    const int64_t stage = (int64_t)tile * kClsTile;
-    for (int r = tid; r < cnt; r += kClsThreads) {
+    const int64_t stage = (int64_t)tile * kStageTile;
+    for (int r = tid; r < cnt; r += 256) {
         mkey[base + r] = stage_key[stage + r];
         midx[base + r] = stage_idx[stage + r];
     }
     const int64_t w0 = stage >> 5, nwords = (n + 31) / 32;
-    for (int w = tid; w < kClsTile / 32 && w0 + w < nwords; w += kClsThreads) mprefix[w0 + w] += base;
+    for (int w = tid; w < kStageTile / 32 && w0 + w < nwords; w += 256) mprefix[w0 + w] += base;
     if (tile == ntiles - 1 && tid == 0) {                // total number of movers, sentinel word
         const uint32_t total = (uint32_t)tile_base[ntiles];
         counters[kCtrMovers] = total;
         counters[kCtrGate] = (2 * (int64_t)total > n) ? 1u : 0u;      // most particles move: reorder before the step kernel
         mask[nwords] = 0u;
         mprefix[nwords] = total;
+        sig->magic = 0;                                  // the emission is used up (the step kernel writes the next one)
     }
 }
 
@@ -344,7 +403,8 @@ k_movers_place(const uint32_t* __restrict__ stage_key, const uint32_t* __restric
 // the counts (C cells instead of one pass over the keys).
 __global__ void __launch_bounds__(kScanThreads) k_scan_cells(const int32_t* __restrict__ count, int32_t* __restrict__ offsets,
                                                               int C, uint32_t* status, uint32_t* tile_counter,
-                                                              uint32_t* __restrict__ digit_hist, int passes, int bits)
+                                                              uint32_t* __restrict__ digit_hist, int passes, int bits,
+                                                              int32_t* __restrict__ offsets2 = nullptr)
 {
     __shared__ uint32_t s_warp[kScanThreads / 32];
     __shared__ uint32_t s_tile, s_excl;
@@ -398,9 +458,15 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_cells(const int32_t* __re
     uint32_t run = s_excl + excl_thread;
 #pragma unroll
     for (int k = 0; k < kScanIPT; ++k) {
-        if (base + k < C) offsets[base + k] = (int32_t)run;
+        if (base + k < C) {
+            offsets[base + k] = (int32_t)run;
+            if (offsets2) offsets2[base + k] = (int32_t)run;
+        }
         run += v[k];
-        if (base + k == C - 1) offsets[C] = (int32_t)run;
+        if (base + k == C - 1) {
+            offsets[C] = (int32_t)run;
+            if (offsets2) offsets2[C] = (int32_t)run;
+        }
     }
     if (digit_hist) {
         for (int i = threadIdx.x; i < passes * kRadix; i += kScanThreads) {
@@ -666,11 +732,12 @@ static int64_t cells_of(const pic_grid_t& g)
 }
 
 struct SortLayout {
-    size_t keys0, keys1, idx0, idx1, pkey, mask, mprefix, old_off, mover_off, cell_base, tile_count, tile_base, lookback;
-    size_t zero_begin, cell_count, mover_count, mover_lo, digit_hist, scan_status, cls_status, counters, zero_end;
-    size_t racc, total;
+    size_t keys0, keys1, idx0, idx1, pkey, mask, mprefix, old_off, prev_off, mover_off, cell_base, tile_count, tile_base, lookback;
+    size_t hist_begin, cell_count, mover_count, mover_lo, hist_end, emit_begin, cell_out, mover_in, emit_end;
+    size_t zero_begin, digit_hist, scan_status, cls_status, counters, zero_end;
+    size_t chain_sig, racc, total;
     int passes, bits, key_bits;
-    int64_t radix_tiles, scan_tiles, cls_tiles;
+    int64_t radix_tiles, scan_tiles, cls_tiles, stage_tiles;
 };
 
 static SortLayout sort_layout(const pic_grid_t& g, int64_t n)
@@ -683,6 +750,7 @@ static SortLayout sort_layout(const pic_grid_t& g, int64_t n)
     L.radix_tiles = (n + kRadixTile - 1) / kRadixTile;
     L.scan_tiles = (C + kScanTile - 1) / kScanTile;
     L.cls_tiles = (n + kClsTile - 1) / kClsTile;
+    L.stage_tiles = (n + kStageTile - 1) / kStageTile;
     size_t off = 0;
     const size_t nb = align256(sizeof(uint32_t) * (size_t)(n > 0 ? n : 1));
     const size_t wb = align256(sizeof(uint32_t) * (size_t)((n + 31) / 32 + 2));
@@ -695,20 +763,28 @@ static SortLayout sort_layout(const pic_grid_t& g, int64_t n)
     L.mask = off; off += wb;
     L.mprefix = off; off += wb;
     L.old_off = off; off += cb;
+    L.prev_off = off; off += cb;
     L.mover_off = off; off += cb;
     L.cell_base = off; off += cb;
-    L.tile_count = off; off += align256(sizeof(int32_t) * (size_t)(L.cls_tiles + 1));
-    L.tile_base = off; off += align256(sizeof(int32_t) * (size_t)(L.cls_tiles + 2));
+    L.tile_count = off; off += align256(sizeof(int32_t) * (size_t)(L.stage_tiles + 1));
+    L.tile_base = off; off += align256(sizeof(int32_t) * (size_t)(L.stage_tiles + 2));
     L.lookback = off; off += align256(sizeof(uint32_t) * (size_t)L.passes * (size_t)(L.radix_tiles > 0 ? L.radix_tiles : 1) * kRadix);
-    L.zero_begin = off;
+    L.hist_begin = off;
     L.cell_count = off; off += cb;
     L.mover_count = off; off += cb;
     L.mover_lo = off; off += cb;
+    L.hist_end = off;
+    L.emit_begin = off;
+    L.cell_out = off; off += cb;
+    L.mover_in = off; off += align256(sizeof(unsigned long long) * (size_t)(C + 1));
+    L.emit_end = off;
+    L.zero_begin = off;
     L.digit_hist = off; off += align256(sizeof(uint32_t) * kMaxPasses * kRadix);
     L.scan_status = off; off += align256(sizeof(uint32_t) * 2 * (size_t)L.scan_tiles);
-    L.cls_status = off; off += align256(sizeof(uint32_t) * (size_t)((L.cls_tiles + kScanTile - 1) / kScanTile + 1));
+    L.cls_status = off; off += align256(sizeof(uint32_t) * (size_t)((L.stage_tiles + kScanTile - 1) / kScanTile + 1));
     L.counters = off; off += 256;
     L.zero_end = off;
+    L.chain_sig = off; off += 256;
     L.racc = off; off += align256(sizeof(double) * (size_t)C);
     L.total = off;
     return L;
@@ -728,6 +804,12 @@ int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, Sor
     o.mask = (uint32_t*)(b + L.mask);
     o.mprefix = (uint32_t*)(b + L.mprefix);
     o.old_off = (int32_t*)(b + L.old_off);
+    o.prev_off = (int32_t*)(b + L.prev_off);
+    o.chain_sig = (ChainSig*)(b + L.chain_sig);
+    o.hist_begin = b + L.hist_begin;
+    o.hist_bytes = L.hist_end - L.hist_begin;
+    o.emit_begin = b + L.emit_begin;
+    o.emit_bytes = L.emit_end - L.emit_begin;
     o.mover_off = (int32_t*)(b + L.mover_off);
     o.cell_base = (int32_t*)(b + L.cell_base);
     o.pkey = (uint32_t*)(b + L.pkey);
@@ -753,34 +835,69 @@ int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, Sor
     o.radix_tiles = L.radix_tiles;
     o.scan_tiles = L.scan_tiles;
     o.cls_tiles = L.cls_tiles;
+    o.stage_tiles = L.stage_tiles;
+    o.emit = EmitP{o.pkey, o.mask, o.mprefix, o.keys[1], o.idx[1], o.tile_count, (int32_t*)(b + L.cell_out),
+                   (unsigned long long*)(b + L.mover_in)};
     return PIC_OK;
+}
+
+// what identifies the particle set `p` on grid g (see ChainSig)
+ChainSig chain_sig_of(const pic_grid_t& g, const pic_particles_t& p)
+{
+    ChainSig s;
+    s.magic = kChainMagic;
+    s.n = (uint64_t)p.n;
+    s.cells = (uint64_t)cells_of(g);
+    uint64_t h = 1469598103934665603ull;                 // FNV-1a over the grid parameters
+    auto mix = [&](uint64_t v) { for (int k = 0; k < 8; ++k) { h ^= (v >> (8 * k)) & 0xFFu; h *= 1099511628211ull; } };
+    mix((uint64_t)g.dim); mix((uint64_t)g.order); mix((uint64_t)g.dtype);
+    for (int c = 0; c < g.dim; ++c) {
+        uint64_t hb;
+        memcpy(&hb, &g.h[c], 8);
+        mix((uint64_t)g.n[c]); mix(hb);
+    }
+    s.grid = h;
+    for (int c = 0; c < 3; ++c) {
+        s.arr[c] = c < g.dim ? (uint64_t)(uintptr_t)p.x[c] : 0;
+        s.arr[3 + c] = c < g.dim ? (uint64_t)(uintptr_t)p.v[c] : 0;
+    }
+    s.arr[6] = (uint64_t)(uintptr_t)p.w;
+    return s;
 }
 
 template <typename T, int D>
 static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_t* perm, int32_t* cell_offsets,
-                          const SortWs& ws, cudaStream_t st)
+                          const SortWs& ws, bool chained, cudaStream_t st)
 {
     const int64_t n = in.n;
     const int C = (int)cells_of(g);
     mark_phase(PIC_PHASE_BEGIN, st);
     PIC_CUDA_OK(cudaMemsetAsync(ws.zero_begin, 0, ws.zero_bytes, st));
-    // the hint: cell_offsets as found on entry
-    k_hint_check<<<(unsigned)((C + 1 + 255) / 256), 256, 0, st>>>(cell_offsets, ws.old_off, C, n, ws.counters);
+    // the hint: cell_offsets as found on entry -- or, in a chain, what the previous step left in the workspace
+    k_hint_check<<<(unsigned)((C + 1 + 255) / 256), 256, 0, st>>>(cell_offsets, ws.prev_off, ws.chain_sig, chain_sig_of(g, in),
+                                                                  chained ? 1 : 0, ws.old_off, C, n, ws.counters);
     count_launch();
     if (n > 0) {
-        // movers are staged per tile in the second halves of the ping-pong arrays, then packed
+        // not a chain: keys, histograms and the stayer/mover split from the positions.  Movers are staged per tile in
+        // the second halves of the ping-pong arrays, then packed
+        k_zero_hist<<<sm_count() * 4, 256, 0, st>>>((uint4*)ws.hist_begin, ws.hist_bytes / 16, ws.counters);
+        k_chain_counts<<<(unsigned)((C + 255) / 256), 256, 0, st>>>(ws.old_off, ws.emit.cell_out, ws.emit.mover_in, ws.cell_count,
+                                                                    ws.mover_count, ws.mover_lo, C, ws.counters);
         k_classify<T, D><<<(unsigned)ws.cls_tiles, kClsThreads, 0, st>>>(
             make_partp<T>(in), make_gridp<T>(g), (int)n, ws.old_off, ws.cell_count, ws.mover_count, ws.mover_lo, ws.keys[1],
             ws.idx[1], ws.mask, ws.mprefix, ws.tile_count, ws.pkey, ws.counters);
-        k_scan_cells<<<(unsigned)((ws.cls_tiles + kScanTile - 1) / kScanTile), kScanThreads, 0, st>>>(
-            ws.tile_count, ws.tile_base, (int)ws.cls_tiles, ws.cls_status, ws.counters + kCtrCls, nullptr, 0, 0);
-        k_movers_place<<<(unsigned)ws.cls_tiles, kClsThreads, 0, st>>>(ws.keys[1], ws.idx[1], ws.keys[0], ws.idx[0], ws.mask,
-                                                                      ws.mprefix, ws.tile_base, (int)ws.cls_tiles, n, ws.counters);
-        count_launch(3);
+        k_scan_cells<<<(unsigned)((ws.stage_tiles + kScanTile - 1) / kScanTile), kScanThreads, 0, st>>>(
+            ws.tile_count, ws.tile_base, (int)ws.stage_tiles, ws.cls_status, ws.counters + kCtrCls, nullptr, 0, 0);
+        k_movers_place<<<(unsigned)ws.stage_tiles, 256, 0, st>>>(ws.keys[1], ws.idx[1], ws.keys[0], ws.idx[0], ws.mask,
+                                                                ws.mprefix, ws.tile_base, (int)ws.stage_tiles, n, ws.counters,
+                                                                ws.chain_sig);
+        count_launch(5);
+    } else {
+        PIC_CUDA_OK(cudaMemsetAsync(ws.hist_begin, 0, ws.hist_bytes, st));
     }
     mark_phase(PIC_PHASE_KEYS, st);
     k_scan_cells<<<(unsigned)ws.scan_tiles, kScanThreads, 0, st>>>(ws.cell_count, cell_offsets, C, ws.scan_status,
-                                                                    ws.counters + kCtrScanA, nullptr, 0, 0);
+                                                                    ws.counters + kCtrScanA, nullptr, 0, 0, ws.prev_off);
     count_launch();
     if (n > 0) {
         k_scan_cells<<<(unsigned)ws.scan_tiles, kScanThreads, 0, st>>>(ws.mover_count, ws.mover_off, C,
@@ -793,12 +910,10 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
         mark_phase(PIC_PHASE_SCAN, st);
         int src = 0;
         for (int q = 0; q < ws.passes; ++q) {
-            const bool last = q == ws.passes - 1;
             k_radix_pass<<<(unsigned)ws.radix_tiles, kRadixThreads, 0, st>>>(
                 ws.keys[src], ws.idx[src], ws.keys[src ^ 1], ws.idx[src ^ 1], ws.counters, q * ws.bits_per_pass,
                 (1u << ws.bits_per_pass) - 1u, ws.digit_hist + q * kRadix, ws.counters + kCtrRadix + q,
                 ws.lookback + (size_t)q * (size_t)pass_stride);
-            (void)last;
             count_launch();
             src ^= 1;
         }
@@ -817,12 +932,20 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
 
 template <typename T, int D>
 static int sort_impl(const pic_grid_t& g, const pic_particles_t& in, pic_particles_t& out, int32_t* perm,
-                     int32_t* cell_offsets, const SortWs& ws, bool reorder, cudaStream_t st)
+                     int32_t* cell_offsets, const SortWs& ws, bool reorder, bool chained, cudaStream_t st)
 {
-    int rc = sort_keys_perm<T, D>(g, in, perm, cell_offsets, ws, st);
+    int rc = sort_keys_perm<T, D>(g, in, perm, cell_offsets, ws, chained, st);
     if (rc != PIC_OK) return rc;
     const int64_t n = in.n;
     if (n > 0 && reorder) return launch_reorder(g, in, out, perm, nullptr, 0u, st);
+    return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+}
+
+// the next call may chain on to the step that has just been enqueued on `out`
+int launch_chain_commit(const pic_grid_t& g, const pic_particles_t& out, const SortWs& ws, cudaStream_t st)
+{
+    k_chain_commit<<<1, 1, 0, st>>>(ws.chain_sig, chain_sig_of(g, out));
+    count_launch();
     return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
 
@@ -846,14 +969,14 @@ int launch_reorder(const pic_grid_t& g, const pic_particles_t& in, const pic_par
 }
 
 int launch_sort(const pic_grid_t& g, const pic_particles_t& in, pic_particles_t& out, int32_t* perm,
-                int32_t* cell_offsets, const SortWs& ws, bool reorder, cudaStream_t st)
+                int32_t* cell_offsets, const SortWs& ws, bool reorder, bool chained, cudaStream_t st)
 {
     if (g.dtype == PIC_F32) {
-        return g.dim == 2 ? sort_impl<float, 2>(g, in, out, perm, cell_offsets, ws, reorder, st)
-                          : sort_impl<float, 3>(g, in, out, perm, cell_offsets, ws, reorder, st);
+        return g.dim == 2 ? sort_impl<float, 2>(g, in, out, perm, cell_offsets, ws, reorder, chained, st)
+                          : sort_impl<float, 3>(g, in, out, perm, cell_offsets, ws, reorder, chained, st);
     }
-    return g.dim == 2 ? sort_impl<double, 2>(g, in, out, perm, cell_offsets, ws, reorder, st)
-                      : sort_impl<double, 3>(g, in, out, perm, cell_offsets, ws, reorder, st);
+    return g.dim == 2 ? sort_impl<double, 2>(g, in, out, perm, cell_offsets, ws, reorder, chained, st)
+                      : sort_impl<double, 3>(g, in, out, perm, cell_offsets, ws, reorder, chained, st);
 }
 
 }  // namespace pic

@@ -19,18 +19,24 @@ static int fused_impl(const pic_grid_t& g, const pic_particles_t& src, pic_parti
     if (perm) {
         // steady state: ONE pass through perm.  Most particles moving (first step, garbage hint): the scattered
         // gather is done by the high-occupancy reorder kernel first and the pass runs in place.  *ws.gate, written
-        // by the sort, selects on the device: the kernels of the other arm return at once.  (Lone particles are
-        // set aside only where the order may be stale: in sorted order they are one-particle cells.)
-        rc = launch_runs<T, D, P, kModeBoth, true>(g, src, p, perm, E, racc, dt, qm, st, ws.gate, 0u);
+        // by the sort, selects on the device: the kernels of the other arm return at once.  Either way the pass
+        // leaves the next sort's inputs behind (EmitP): the counters it adds to are zero from here on.
+        PIC_CUDA_OK(cudaMemsetAsync(ws.emit_begin, 0, ws.emit_bytes, st));
+        rc = launch_runs<T, D, P, kModeBoth, true>(g, src, p, perm, E, racc, dt, qm, st, ws.gate, 0u, nullptr, nullptr, &ws.emit);
         if (rc != PIC_OK) return rc;
         if ((rc = launch_reorder(g, src, p, perm, ws.gate, 1u, st)) != PIC_OK) return rc;
-        rc = launch_runs<T, D, P, kModeBoth, false>(g, p, p, nullptr, E, racc, dt, qm, st, ws.gate, 1u, ws.stray_list, ws.stray_count);
+        rc = launch_runs<T, D, P, kModeBoth, false>(g, p, p, nullptr, E, racc, dt, qm, st, ws.gate, 1u, nullptr, nullptr, &ws.emit);
+        if (rc != PIC_OK) return rc;
+        if (p.n > 0 && (rc = launch_chain_commit(g, p, ws, st)) != PIC_OK) return rc;
     } else {
+        // the order of an earlier sort, in place: lone particles (drifted since) are set aside for k_strays.  The
+        // positions change under the workspace's emission, if any: it is void from here on
+        PIC_CUDA_OK(cudaMemsetAsync(ws.chain_sig, 0, sizeof(ChainSig), st));
         PIC_CUDA_OK(cudaMemsetAsync(ws.stray_count, 0, sizeof(uint32_t), st));
         rc = launch_runs<T, D, P, kModeBoth, false>(g, p, p, nullptr, E, racc, dt, qm, st, nullptr, 0u, ws.stray_list, ws.stray_count);
+        if (rc != PIC_OK) return rc;
+        if ((rc = launch_strays<T, D, P, kModeBoth>(g, p, E, racc, dt, qm, ws.stray_list, ws.stray_count, sm_count(), st)) != PIC_OK) return rc;
     }
-    if (rc != PIC_OK) return rc;
-    if ((rc = launch_strays<T, D, P, kModeBoth>(g, p, E, racc, dt, qm, ws.stray_list, ws.stray_count, sm_count(), st)) != PIC_OK) return rc;
     if (sizeof(T) == 4) {
         k_round_rho<T><<<(unsigned)((C + 255) / 256), 256, 0, st>>>(racc, (T*)rho, C);
         count_launch();

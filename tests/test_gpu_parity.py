@@ -542,3 +542,106 @@ def test_step_fields_host_entry_point():
     with pytest.raises(B.PicError, match="workspace"):
         B.pic_step_fields_host(gb, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], perm, off, rho, wl.E,
                                cfg.dt, cfg.qm, True, ws[: 4096])
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# PIC_SORT_CHAINED (row a8: the step kernel emits the next step's keys, histogram and mover list).  The chained
+# sort must give, bit for bit, what the sort from the positions gives; the latter is compared with the oracle in
+# lockstep above, the former also directly below.
+CHAIN_CASES = [
+    ("cfg2", dict(N=200_003, n=(64, 64))),
+    ("cfg3", dict(N=150_001, n=(32, 32, 32))),
+    ("cfg3", dict(N=3 * 2048 + 1, n=(8, 8, 8))),
+    ("cfg4", dict(N=300_007, n=(32, 32, 32))),
+    ("cfg5", dict(N=8 * 16 ** 3 + 5, n=(16, 16, 16))),
+    ("cfg1", dict()),
+]
+
+
+def _same_state(a, b, n, cells, what):
+    assert torch.equal(a.perm[:n], b.perm[:n]), "perm, " + what
+    assert torch.equal(a.cell_offsets[: cells + 1], b.cell_offsets[: cells + 1]), "cell_offsets, " + what
+    for c in range(len(a.cur["x"])):
+        assert torch.equal(a.cur["x"][c], b.cur["x"][c]), "x[%d], %s" % (c, what)
+        assert torch.equal(a.cur["v"][c], b.cur["v"][c]), "v[%d], %s" % (c, what)
+    assert torch.equal(a.cur["w"], b.cur["w"]), "w, " + what
+
+
+@pytest.mark.parametrize("name,kw", CHAIN_CASES)
+def test_chained_steps_equal_unchained_bit_for_bit(name, kw):
+    O, B = _mods()
+    cfg = _cfg(name, kw)
+    wl = W.make_workload(cfg)
+    g = B.grid_of(cfg)
+    a = B.Stepper(g, wl.x, wl.v, wl.w, wl.E)
+    b = B.Stepper(g, wl.x, wl.v, wl.w, wl.E)
+    # sorted steps, an unsorted one in between (which breaks the chain), sorted steps again
+    plan = [True, True, True, False, True, True, True, True]
+    for k, do_sort in enumerate(plan):
+        a.step(cfg.dt, cfg.qm, do_sort, chained=True)
+        b.step(cfg.dt, cfg.qm, do_sort, chained=False)
+        torch.cuda.synchronize()
+        if do_sort:
+            _same_state(a, b, cfg.N, g.cells, "step %d" % k)
+        ra, rb = a.rho.double(), b.rho.double()
+        assert float((ra - rb).abs().max()) <= TOL_RHO[cfg.dtype] * float(rb.abs().max()), "rho, step %d" % k
+
+
+@pytest.mark.parametrize("name,kw", [("cfg3", dict(N=150_001, n=(32, 32, 32))), ("cfg5", dict(N=8 * 16 ** 3 + 5, n=(16, 16, 16)))])
+def test_chained_steps_against_oracle_lockstep_by_id(name, kw):
+    """A free-running chained GPU run and the oracle, step by step: while no particle sits within rounding of a cell
+    face the two orders are identical, and then perm and cell_offsets must agree bit for bit at every step."""
+    O, B = _mods()
+    cfg = _cfg(name, kw)
+    wl = W.make_workload(cfg)
+    go, g = O.grid_of(cfg), B.grid_of(cfg)
+    st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E)
+    x, v, w = wl.x, wl.v, wl.w
+    for k in range(6):
+        # the oracle steps from the GPU's own state: the chain is not touched (nothing is written to the device)
+        st.step(cfg.dt, cfg.qm, True, chained=True)
+        r = O.step(go, x, v, w, wl.E, cfg.dt, cfg.qm)
+        torch.cuda.synchronize()
+        assert np.array_equal(st.perm[: cfg.N].cpu().numpy(), r["perm"]), "perm, step %d" % k
+        assert np.array_equal(st.cell_offsets[: g.cells + 1].cpu().numpy(), r["cell_offsets"]), "cell_offsets, step %d" % k
+        assert err_rho(st.rho.cpu().numpy(), r["rho"]) <= TOL_RHO[cfg.dtype]
+        x = [a.cpu().numpy() for a in st.cur["x"]]
+        v = [a.cpu().numpy() for a in st.cur["v"]]
+        w = st.cur["w"].cpu().numpy()
+        for c in range(cfg.dim):
+            assert err_x(x[c], r["x"][c], cfg.L[c]) <= TOL_XV[cfg.dtype]
+            assert err_v(v[c], r["v"][c]) <= TOL_XV[cfg.dtype]
+
+
+def test_chain_flag_on_foreign_arrays_falls_back():
+    """PIC_SORT_CHAINED on arrays the workspace's emission does not belong to (other addresses, another sort in
+    between) must behave like PIC_SORT: the device-side check of the chain signature."""
+    O, B = _mods()
+    cfg = _cfg("cfg3", dict(N=60_001, n=(16, 16, 16)))
+    wl = W.make_workload(cfg)
+    go, g = O.grid_of(cfg), B.grid_of(cfg)
+    n = cfg.N
+    st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E)
+    st.step(cfg.dt, cfg.qm, True)
+    st.step(cfg.dt, cfg.qm, True)
+    torch.cuda.synchronize()
+    # (1) other arrays, same workspace, chained flag
+    wl2 = W.make_workload(cfg.scaled(n, seed=cfg.seed + 7))
+    ref = O.step(go, wl2.x, wl2.v, wl2.w, wl2.E, cfg.dt, cfg.qm)
+    x, v, w = to_dev(wl2.x), to_dev(wl2.v), to_dev([wl2.w])[0]
+    xo, vo, wo = [torch.empty_like(a) for a in x], [torch.empty_like(a) for a in v], torch.empty_like(w)
+    E = to_dev(wl2.E)
+    B.pic_step(g, x, v, w, xo, vo, wo, st.perm, st.cell_offsets, st.rho, E, cfg.dt, cfg.qm, B.PIC_SORT_CHAINED, st.ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(st.perm[:n].cpu().numpy(), ref["perm"])
+    assert np.array_equal(st.cell_offsets[: g.cells + 1].cpu().numpy(), ref["cell_offsets"])
+    # (2) that call has left an emission for (xo, vo, wo); a pic_sort on the same workspace voids it
+    perm2 = torch.empty_like(st.perm)
+    off2 = torch.zeros_like(st.cell_offsets)
+    B.pic_sort(g, x, v, w, [torch.empty_like(a) for a in x], [torch.empty_like(a) for a in v], torch.empty_like(w), perm2, off2, st.ws)
+    ref2 = O.step(go, to_host(xo), to_host(vo), wo.cpu().numpy(), wl2.E, cfg.dt, cfg.qm)   # from the GPU's own state
+    x2, v2, w2 = [torch.empty_like(a) for a in x], [torch.empty_like(a) for a in v], torch.empty_like(w)
+    B.pic_step(g, xo, vo, wo, x2, v2, w2, st.perm, st.cell_offsets, st.rho, E, cfg.dt, cfg.qm, B.PIC_SORT_CHAINED, st.ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(st.cell_offsets[: g.cells + 1].cpu().numpy(), ref2["cell_offsets"])
+    assert np.array_equal(st.perm[:n].cpu().numpy(), ref2["perm"])
