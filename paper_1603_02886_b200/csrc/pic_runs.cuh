@@ -180,7 +180,8 @@ __global__ void __launch_bounds__(128) k_strays(PartP<T> p, GridP<T> g, FieldP<T
 
 // STRAYS: lone particles are set aside in stray_list for k_strays (used where the order may be stale)
 // EMIT:   the next sort's inputs are written as the particles are pushed (sorted input only: !STRAYS)
-template <typename T, int D, int P, int MODE, bool VIA_PERM, int G_, bool STRAYS, bool EMIT>
+// HM:     every spacing is a power of two, so x/h is the product x * (1/h) bit for bit (R13): no division path
+template <typename T, int D, int P, int MODE, bool VIA_PERM, int G_, bool STRAYS, bool EMIT, bool HM>
 __global__ void PIC_RUNS_BOUNDS(T)
 k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g, FieldP<T> f, int64_t n,
        double* __restrict__ racc, double dtd, double qmdtd, const uint32_t* __restrict__ gate, uint32_t want,
@@ -191,6 +192,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
     using SH = RunsShape<T, D, P, G_>;
     if (gate && *gate != want) return;                // the other arm of a device-side choice runs instead
     const T dt = (T)dtd, qmdt = (T)qmdtd;
+    const int hm = HM ? 1 : g.hmul;
     constexpr int S = SH::S, S2 = S / 2, SZ = SH::SZ, ROWS = SH::ROWS;
     constexpr int G = SH::G, RPL = SH::RPL, NG = SH::NG, NV = SH::NV, NODES = SH::NODES, NPL = SH::NPL;
     constexpr int WR = SH::WR, RECS = SH::RECS;
@@ -401,10 +403,10 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
         bool lonely = false;
         auto write_record = [&]() {
             T w1[S], w2[S], w3[SZ];
-            const int cx = cell_weights<T, P>(px[0], g.h[0], g.inv_h[0], g.hmul, g.n[0], w1);
-            const int cy = cell_weights<T, P>(px[1], g.h[1], g.inv_h[1], g.hmul, g.n[1], w2);
+            const int cx = cell_weights<T, P>(px[0], g.h[0], g.inv_h[0], hm, g.n[0], w1);
+            const int cy = cell_weights<T, P>(px[1], g.h[1], g.inv_h[1], hm, g.n[1], w2);
             int cz = 0;
-            if constexpr (D == 3) cz = cell_weights<T, P>(px[2], g.h[2], g.inv_h[2], g.hmul, g.n[2], w3);
+            if constexpr (D == 3) cz = cell_weights<T, P>(px[2], g.h[2], g.inv_h[2], hm, g.n[2], w3);
             if constexpr (!STRAYS) {
                 c0 = cx; c1 = cy; c2 = cz;
                 if (valid) key = c0 + g.n[0] * (c1 + g.n[1] * c2);
@@ -417,9 +419,9 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
             if constexpr (DEP) sts1<T>(a_q + (uint32_t)idx * B, (valid && !lonely) ? pw * g.inv_vol : (T)0);
         };
         if constexpr (STRAYS) {
-            c0 = cell_index(grid_coord(px[0], g.h[0], g.inv_h[0], g.hmul), g.n[0]);
-            c1 = cell_index(grid_coord(px[1], g.h[1], g.inv_h[1], g.hmul), g.n[1]);
-            if constexpr (D == 3) c2 = cell_index(grid_coord(px[2], g.h[2], g.inv_h[2], g.hmul), g.n[2]);
+            c0 = cell_index(grid_coord(px[0], g.h[0], g.inv_h[0], hm), g.n[0]);
+            c1 = cell_index(grid_coord(px[1], g.h[1], g.inv_h[1], hm), g.n[1]);
+            if constexpr (D == 3) c2 = cell_index(grid_coord(px[2], g.h[2], g.inv_h[2], hm), g.n[2]);
             if (valid) key = c0 + g.n[0] * (c1 + g.n[1] * c2);
             // a particle whose key differs from both neighbours' is a STRAY: it does not break the run around it but
             // is set aside for k_strays.  The others are the RECORDS of the batch, in order.
@@ -556,7 +558,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
             int nk = 0, mul = 1;
 #pragma unroll
             for (int c = 0; c < D; ++c) {
-                nk += mul * cell_index(grid_coord(px[c], g.h[c], g.inv_h[c], g.hmul), g.n[c]);
+                nk += mul * cell_index(grid_coord(px[c], g.h[c], g.inv_h[c], hm), g.n[c]);
                 mul *= g.n[c];
             }
             const bool mover = valid && nk != key;
@@ -606,30 +608,20 @@ inline int launch_runs(const pic_grid_t& g, const pic_particles_t& src, const pi
     constexpr int64_t per_block = (int64_t)SH::WR * kRunsWarps;
     const unsigned blocks = (unsigned)((dst.n + per_block - 1) / per_block);
     const EmitP none{};
-    if constexpr (MODE == kModeBoth) {
-        if (emit) {
-            auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, false, true>;
-            kern<<<blocks, kRunsThreads, smem, st>>>(make_partp<T>(VIA_PERM ? src : dst), make_partp<T>(dst), perm,
-                                                    make_gridp<T>(g), f, dst.n, racc, dt, qm * dt, gate, want,
-                                                    nullptr, nullptr, *emit);
-            count_launch();
-            return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
-        }
-    }
-    if (stray_list && stray_count) {
-        auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, true, false>;
-        kern<<<blocks, kRunsThreads, smem, st>>>(make_partp<T>(VIA_PERM ? src : dst), make_partp<T>(dst), perm,
-                                                make_gridp<T>(g), f, dst.n, racc, dt, qm * dt, gate, want,
-                                                stray_list, stray_count, none);
+    const GridP<T> gp = make_gridp<T>(g);
+    const PartP<T> ps = make_partp<T>(VIA_PERM ? src : dst), pd = make_partp<T>(dst);
+    auto go = [&](auto kern, uint32_t* sl, uint32_t* sc, const EmitP& em) {
+        kern<<<blocks, kRunsThreads, smem, st>>>(ps, pd, perm, gp, f, dst.n, racc, dt, qm * dt, gate, want, sl, sc, em);
         count_launch();
         return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+    };
+    if constexpr (MODE == kModeBoth) {
+        if (emit)
+            return gp.hmul ? go(k_runs<T, D, P, MODE, VIA_PERM, GP, false, true, true>, nullptr, nullptr, *emit)
+                           : go(k_runs<T, D, P, MODE, VIA_PERM, GP, false, true, false>, nullptr, nullptr, *emit);
     }
-    auto kern = k_runs<T, D, P, MODE, VIA_PERM, GP, false, false>;
-    kern<<<blocks, kRunsThreads, smem, st>>>(make_partp<T>(VIA_PERM ? src : dst), make_partp<T>(dst), perm,
-                                            make_gridp<T>(g), f, dst.n, racc, dt, qm * dt, gate, want,
-                                            stray_list, stray_count, none);
-    count_launch();
-    return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+    if (stray_list && stray_count) return go(k_runs<T, D, P, MODE, VIA_PERM, GP, true, false, false>, stray_list, stray_count, none);
+    return go(k_runs<T, D, P, MODE, VIA_PERM, GP, false, false, false>, nullptr, nullptr, none);
 }
 
 // the particles k_runs has set aside, in place on p

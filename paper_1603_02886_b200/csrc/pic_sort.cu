@@ -27,7 +27,7 @@
 //           k_scan_digits    digit histograms -> exclusive global digit offsets
 //           k_radix_pass     one stable partition of the movers by an (at most) 8-bit digit
 //           k_cell_base      per cell: where its stayers start in perm
-//           k_perm_movers / k_perm_stayers   perm
+//           k_perm_stayers   perm of the stayers (the movers' entries come from the last radix pass)
 //           k_reorder        out_a[j] = in_a[perm[j]] for every attribute (pic_sort only)
 #include <cmath>
 #include <cstring>
@@ -286,7 +286,7 @@ template <typename T, int D>
 #ifndef PIC_CLS_MINB
 #define PIC_CLS_MINB 4
 #endif
-__global__ void __launch_bounds__(kClsThreads, PIC_CLS_MINB)
+__global__ void __launch_bounds__(kClsThreads, (sizeof(T) == 8 ? PIC_CLS_MINB / 2 : PIC_CLS_MINB))   // (doubles: 64 registers spill)
 k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, int32_t* __restrict__ cell_count,
            int32_t* __restrict__ mover_count, int32_t* __restrict__ mover_lo, uint32_t* __restrict__ mkey,
            uint32_t* __restrict__ midx, uint32_t* __restrict__ mask, uint32_t* __restrict__ mprefix,
@@ -514,11 +514,21 @@ __global__ void __launch_bounds__(256) k_zero_lookback(uint32_t* lookback, const
 #ifndef PIC_RADIX_MINB
 #define PIC_RADIX_MINB 5        // resident blocks per SM k_radix_pass is compiled for (48 registers)
 #endif
+// LAST: the pairs leave this pass sorted by (key, position), so the place of each in perm is known here and the
+// sorted list is never written: the r-th mover of key k goes below the stayers of k if it comes from below the
+// hint interval of k, else above them.
+struct PermP {
+    const int32_t* new_off;      // [C+1] cell_offsets of this sort
+    const int32_t* mover_off;    // [C+1] exclusive scan of the movers' histogram
+    const int32_t* old_off;      // [C+1] the hint
+    int32_t* perm;
+};
+template <bool LAST>
 __global__ void __launch_bounds__(kRadixThreads, PIC_RADIX_MINB)
 k_radix_pass(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ idx_in,
              uint32_t* __restrict__ keys_out, uint32_t* __restrict__ idx_out, const uint32_t* __restrict__ counters,
              int shift, uint32_t mask, const uint32_t* __restrict__ digit_offsets, uint32_t* tile_counter,
-             uint32_t* lookback)
+             uint32_t* lookback, PermP pp)
 {
     __shared__ uint32_t s_cnt[kRadixWarps][kRadix];   // per-warp digit counters -> per-warp bases
     __shared__ uint32_t s_start[kRadix];              // tile-local start of each digit
@@ -620,11 +630,21 @@ k_radix_pass(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ 
     }
     __syncthreads();
     // coalesced write-out: consecutive local positions of one digit are consecutive in global memory
+    const bool hint_ok = counters[kCtrHintBad] == 0u;
     for (int q = tid; q < tile_valid; q += kRadixThreads) {
         uint32_t k = s_keys[q];
         uint32_t dst = s_base[(k >> shift) & mask] + q;
-        if (keys_out) keys_out[dst] = k;
-        idx_out[dst] = s_idx[q];
+        if constexpr (LAST) {
+            const int32_t i = (int32_t)s_idx[q];
+            const int32_t m0 = pp.mover_off[k], m1 = pp.mover_off[k + 1];
+            const int32_t n0 = pp.new_off[k], n1 = pp.new_off[k + 1];
+            const int32_t stay = (n1 - n0) - (m1 - m0);
+            const bool below = hint_ok && i < pp.old_off[k];
+            pp.perm[n0 + ((int32_t)dst - m0) + (below ? 0 : stay)] = i;
+        } else {
+            keys_out[dst] = k;
+            idx_out[dst] = s_idx[q];
+        }
     }
 }
 
@@ -642,26 +662,6 @@ __global__ void __launch_bounds__(256) k_cell_base(const int32_t* __restrict__ n
     const int32_t a = old_off[k];
     const uint32_t mv = mprefix[a >> 5] + __popc(mask[a >> 5] & ((1u << (a & 31)) - 1u));
     cell_base[k] = new_off[k] + mover_lo[k] - a + (int32_t)mv;
-}
-
-// movers, sorted by (key, position): the r-th mover of key k goes below the stayers if it comes
-// from below the hint interval of k, else above them
-__global__ void __launch_bounds__(256) k_perm_movers(const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
-                                                     const int32_t* __restrict__ new_off, const int32_t* __restrict__ mover_off,
-                                                     const int32_t* __restrict__ old_off, int32_t* __restrict__ perm,
-                                                     const uint32_t* __restrict__ counters)
-{
-    const int64_t nm = counters[kCtrMovers];
-    const bool hint_ok = counters[kCtrHintBad] == 0u;
-    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < nm; q += (int64_t)gridDim.x * blockDim.x) {
-        const int k = (int)skey[q];
-        const int32_t i = (int32_t)sidx[q];
-        const int32_t m0 = mover_off[k], m1 = mover_off[k + 1];
-        const int32_t n0 = new_off[k], n1 = new_off[k + 1];
-        const int32_t stay = (n1 - n0) - (m1 - m0);
-        const bool below = hint_ok && i < old_off[k];
-        perm[n0 + ((int32_t)q - m0) + (below ? 0 : stay)] = i;
-    }
 }
 
 // stayers: position i (mover bit clear) kept its cell k = pkey[i] and goes to
@@ -909,22 +909,22 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
         count_launch(3);
         mark_phase(PIC_PHASE_SCAN, st);
         int src = 0;
+        const PermP pp{cell_offsets, ws.mover_off, ws.old_off, perm};
         for (int q = 0; q < ws.passes; ++q) {
-            k_radix_pass<<<(unsigned)ws.radix_tiles, kRadixThreads, 0, st>>>(
+            auto kern = (q == ws.passes - 1) ? k_radix_pass<true> : k_radix_pass<false>;
+            kern<<<(unsigned)ws.radix_tiles, kRadixThreads, 0, st>>>(
                 ws.keys[src], ws.idx[src], ws.keys[src ^ 1], ws.idx[src ^ 1], ws.counters, q * ws.bits_per_pass,
                 (1u << ws.bits_per_pass) - 1u, ws.digit_hist + q * kRadix, ws.counters + kCtrRadix + q,
-                ws.lookback + (size_t)q * (size_t)pass_stride);
+                ws.lookback + (size_t)q * (size_t)pass_stride, pp);
             count_launch();
             src ^= 1;
         }
         mark_phase(PIC_PHASE_RADIX, st);
         k_cell_base<<<(unsigned)((C + 255) / 256), 256, 0, st>>>(cell_offsets, ws.old_off, ws.mover_lo, ws.mask, ws.mprefix,
                                                                  ws.cell_base, C, ws.counters);
-        k_perm_movers<<<sm_count() * 8, 256, 0, st>>>(ws.keys[src], ws.idx[src], cell_offsets, ws.mover_off, ws.old_off, perm,
-                                              ws.counters);
         k_perm_stayers<<<(unsigned)((n + 256 * kStayIPT - 1) / (256 * kStayIPT)), 256, 0, st>>>(
             ws.pkey, ws.cell_base, ws.mask, ws.mprefix, perm, (int)n, ws.counters);
-        count_launch(3);
+        count_launch(2);
     }
     mark_phase(PIC_PHASE_REORDER, st);
     return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
