@@ -180,6 +180,51 @@ def sort(g: Grid, x, v, w):
     return xo, vo, wo, perm, off
 
 
+def _bucket3(g: Grid, bucket):
+    b = (ctypes.c_int32 * 3)(1, 1, 1)
+    for c in range(g.dim):
+        b[c] = int(bucket[c])
+    return b
+
+
+def bucket_count(g: Grid, bucket) -> int:
+    """Number of buckets of `bucket[c]` cells per dimension (NEXT-2)."""
+    cg = g.c()
+    lib = _load()
+    lib.pic_ref_bucket_count.restype = ctypes.c_int64
+    B = lib.pic_ref_bucket_count(ctypes.byref(cg), _bucket3(g, bucket))
+    if B < 0:
+        _rc(-1)
+    return int(B)
+
+
+def bucket_keys(g: Grid, x, bucket) -> np.ndarray:
+    n = x[0].shape[0]
+    _chk(g, x, n)
+    key = np.empty(n, np.int32)
+    cg = g.c()
+    _rc(_load().pic_ref_bucket_keys(ctypes.byref(cg), _bucket3(g, bucket), ctypes.c_int64(n), _ptrs(x),
+                                    ctypes.c_void_p(key.ctypes.data)))
+    return key
+
+
+def sort_buckets(g: Grid, x, v, w, bucket):
+    """Stable sort by bucket key -> (x_out, v_out, w_out, perm[n] int32, bucket_offsets[B+1] int32)."""
+    n = w.shape[0]
+    _chk(g, list(x) + list(v) + [w], n)
+    xo = [np.empty_like(a) for a in x]
+    vo = [np.empty_like(a) for a in v]
+    wo = np.empty_like(w)
+    perm = np.empty(n, np.int32)
+    off = np.empty(bucket_count(g, bucket) + 1, np.int32)
+    cg = g.c()
+    _rc(_load().pic_ref_sort_buckets(ctypes.byref(cg), _bucket3(g, bucket), ctypes.c_int64(n), _ptrs(x), _ptrs(v),
+                                     ctypes.c_void_p(w.ctypes.data), _ptrs(xo), _ptrs(vo),
+                                     ctypes.c_void_p(wo.ctypes.data), ctypes.c_void_p(perm.ctypes.data),
+                                     ctypes.c_void_p(off.ctypes.data)))
+    return xo, vo, wo, perm, off
+
+
 def deposit(g: Grid, x, w, allpairs: bool = False) -> np.ndarray:
     """rho[C] in float64, x fastest."""
     n = w.shape[0]

@@ -242,6 +242,84 @@ int pic_ref_sort(const pic_ref_grid *g, int64_t n,
 }
 
 /* ---------------------------------------------------------------------------
+ * NEXT-2. Buckets of several cells (section 3.2: "a bucket ... one or more grid
+ * cells"; App. B: "ibin = bin % nsplitx; jbin = bin / nsplitx", bins ordered x
+ * fastest; the bucket-count sweep of PAPER.md:336-350 Fig. 9 and 396-402 Fig. 14).
+ * A bucket is a box of bucket[c] cells per dimension (the last one of a dimension is smaller
+ * when bucket[c] does not divide n[c]); there are nb[c] = ceil(n[c] / bucket[c]) per dimension.
+ *   key_i = b_x + nb_x (b_y + nb_y b_z),  b_c = floor(cell_c / bucket[c]),
+ * cell_c the clamped cell index of a1.  The sort is the same stable counting sort with this
+ * key: particles of one bucket become contiguous and keep their source order inside it (the
+ * paper leaves that order arbitrary).  bucket = (1,1,1) is pic_ref_sort.
+ * ------------------------------------------------------------------------- */
+static int bucket_ok(const pic_ref_grid *g, const int32_t bucket[3])
+{
+    for (int c = 0; c < g->dim; ++c)
+        if (bucket[c] < 1 || bucket[c] > g->n[c]) return 0;
+    return 1;
+}
+
+int64_t pic_ref_bucket_count(const pic_ref_grid *g, const int32_t bucket[3])
+{
+    if (!grid_ok(g) || !bucket_ok(g, bucket)) return -1;
+    int64_t B = 1;
+    for (int c = 0; c < g->dim; ++c) B *= (g->n[c] + bucket[c] - 1) / bucket[c];
+    return B;
+}
+
+static int32_t bucket_key(const pic_ref_grid *g, const int32_t bucket[3], const void *const x[3], int64_t i)
+{
+    int64_t key = 0, stride = 1;
+    for (int c = 0; c < g->dim; ++c) {
+        int32_t cell = cell_index(g, c, grid_coord(g, c, x[c], i));
+        key += stride * (cell / bucket[c]);
+        stride *= (g->n[c] + bucket[c] - 1) / bucket[c];
+    }
+    return (int32_t)key;
+}
+
+int pic_ref_bucket_keys(const pic_ref_grid *g, const int32_t bucket[3], int64_t n, const void *const x[3], int32_t *key)
+{
+    if (!grid_ok(g) || !bucket_ok(g, bucket) || n < 0) return REF_BAD_ARG;
+    for (int64_t i = 0; i < n; ++i) key[i] = bucket_key(g, bucket, x, i);
+    return REF_OK;
+}
+
+int pic_ref_sort_buckets(const pic_ref_grid *g, const int32_t bucket[3], int64_t n,
+                         const void *const xin[3], const void *const vin[3], const void *win,
+                         void *const xout[3], void *const vout[3], void *wout,
+                         int32_t *perm, int32_t *bucket_offsets)
+{
+    if (!grid_ok(g) || !bucket_ok(g, bucket) || n < 0 || n > 2147483647LL) return REF_BAD_ARG;
+    int64_t B = pic_ref_bucket_count(g, bucket);
+    int32_t *key = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+    int32_t *cursor = (int32_t *)malloc(sizeof(int32_t) * (size_t)(B + 1));
+    if (!key || !cursor) { free(key); free(cursor); return REF_BAD_ARG; }
+    for (int64_t k = 0; k <= B; ++k) bucket_offsets[k] = 0;
+    for (int64_t i = 0; i < n; ++i) {                    /* histogram */
+        key[i] = bucket_key(g, bucket, xin, i);
+        bucket_offsets[key[i] + 1] += 1;
+    }
+    for (int64_t k = 0; k < B; ++k)                      /* prefix sum */
+        bucket_offsets[k + 1] += bucket_offsets[k];
+    for (int64_t k = 0; k < B; ++k) cursor[k] = bucket_offsets[k];
+    for (int64_t i = 0; i < n; ++i)                      /* stable scatter */
+        perm[cursor[key[i]]++] = (int32_t)i;
+    size_t s = g->dtype ? 8 : 4;
+    for (int64_t j = 0; j < n; ++j) {                    /* move the attributes bit for bit */
+        int64_t i = perm[j];
+        for (int c = 0; c < g->dim; ++c) {
+            memcpy((char *)xout[c] + s * j, (const char *)xin[c] + s * i, s);
+            memcpy((char *)vout[c] + s * j, (const char *)vin[c] + s * i, s);
+        }
+        memcpy((char *)wout + s * j, (const char *)win + s * i, s);
+    }
+    free(key);
+    free(cursor);
+    return REF_OK;
+}
+
+/* ---------------------------------------------------------------------------
  * O3 / a5. Charge deposit (setrho, threads-on-particles form without the threads:
  * PAPER.md:292-294 section 3.3.4; the 8 products of PAPER.md:509-519 for p = 1).
  *   rho[j] = h^-d sum_i w_i prod_c W_p(x_ic/h_c - j_c)   on the periodic grid.

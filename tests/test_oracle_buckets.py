@@ -1,0 +1,96 @@
+"""Pins of the oracle's bucket sort (NEXT-2: buckets of several cells):
+a hand-written numpy key with numpy's stable argsort, the special cases that reduce to the
+cell sort and to the identity, and the invariants of a stable counting sort."""
+import numpy as np
+import pytest
+
+import oracle as O
+import pic_workloads as W
+
+
+def cfg_of(dim, dtype, N, n, seed=0):
+    return W.Config("t", dim, tuple(n), N, dtype, 1, "uniform", 3, 1, seed=seed)
+
+
+def numpy_bucket_key(cfg, x, bucket):
+    """b_c = floor(cell_c / bucket_c), key = b_x + nb_x (b_y + nb_y b_z): bins x fastest."""
+    key = np.zeros(cfg.N, np.int64)
+    stride = 1
+    for c in range(cfg.dim):
+        cell = np.clip(np.floor(x[c] / cfg.np_dtype(cfg.h)).astype(np.int64), 0, cfg.n[c] - 1)
+        key += stride * (cell // bucket[c])
+        stride *= -(-cfg.n[c] // bucket[c])
+    return key, stride
+
+
+CASES = [
+    (2, "f64", (16, 16), (4, 2)),
+    (2, "f32", (32, 16), (16, 16)),      # the paper's 512x256 grid in 32x16 buckets, scaled down
+    (3, "f32", (8, 8, 8), (2, 2, 2)),
+    (3, "f64", (8, 8, 8), (4, 4, 4)),
+    (3, "f64", (10, 6, 7), (3, 4, 2)),   # bucket sizes that do not divide the grid: ragged last buckets
+    (3, "f32", (8, 8, 8), (8, 1, 1)),    # whole x rows
+]
+
+
+@pytest.mark.parametrize("dim,dtype,n,bucket", CASES)
+def test_bucket_sort_equals_numpy_stable_argsort(dim, dtype, n, bucket):
+    cfg = cfg_of(dim, dtype, 20011, n)
+    wl = W.make_workload(cfg)
+    g = O.grid_of(cfg)
+    key, B = numpy_bucket_key(cfg, wl.x, bucket)
+    assert O.bucket_count(g, bucket) == B
+    assert np.array_equal(O.bucket_keys(g, wl.x, bucket), key.astype(np.int32))
+    xo, vo, wo, perm, off = O.sort_buckets(g, wl.x, wl.v, wl.w, bucket)
+    assert np.array_equal(perm, np.argsort(key, kind="stable").astype(np.int32))
+    assert np.array_equal(off, np.concatenate([[0], np.cumsum(np.bincount(key, minlength=B))]).astype(np.int32))
+    assert np.array_equal(np.sort(perm), np.arange(cfg.N, dtype=np.int32))
+    ks = key[perm]
+    assert np.all(np.diff(ks) >= 0)
+    assert np.all(np.diff(perm.astype(np.int64))[np.diff(ks) == 0] > 0)      # ties keep the source order
+    for c in range(dim):
+        assert np.array_equal(xo[c], wl.x[c][perm]) and np.array_equal(vo[c], wl.v[c][perm])
+    assert np.array_equal(wo, wl.w[perm])
+
+
+@pytest.mark.parametrize("dim,n", [(2, (16, 16)), (3, (8, 8, 8))])
+def test_unit_buckets_are_the_cell_sort_and_one_bucket_is_the_identity(dim, n):
+    cfg = cfg_of(dim, "f64", 7001, n, seed=3)
+    wl = W.make_workload(cfg)
+    g = O.grid_of(cfg)
+    ones = (1,) * dim
+    a = O.sort(g, wl.x, wl.v, wl.w)
+    b = O.sort_buckets(g, wl.x, wl.v, wl.w, ones)
+    assert np.array_equal(a[3], b[3]) and np.array_equal(a[4], b[4])
+    assert np.array_equal(O.keys(g, wl.x), O.bucket_keys(g, wl.x, ones))
+    # one bucket holding the whole grid: nothing moves
+    _, _, _, perm, off = O.sort_buckets(g, wl.x, wl.v, wl.w, n)
+    assert np.array_equal(perm, np.arange(cfg.N, dtype=np.int32))
+    assert np.array_equal(off, np.array([0, cfg.N], np.int32))
+
+
+def test_bucket_order_refines_to_cell_order():
+    """Sorting by cell inside every bucket of a bucket-sorted array gives, bucket by bucket, the same particle
+    sets as the cell sort restricted to the cells of that bucket (a bucket is a union of cells)."""
+    cfg = cfg_of(3, "f32", 30011, (8, 8, 8), seed=5)
+    wl = W.make_workload(cfg)
+    g = O.grid_of(cfg)
+    bucket = (4, 2, 2)
+    _, _, _, perm_b, off_b = O.sort_buckets(g, wl.x, wl.v, wl.w, bucket)
+    cell = O.keys(g, wl.x)
+    bkey = O.bucket_keys(g, wl.x, bucket)
+    for k in range(off_b.size - 1):
+        ids = perm_b[off_b[k]: off_b[k + 1]]
+        assert np.all(bkey[ids] == k)
+        cx, cy, cz = cell[ids] % 8, (cell[ids] // 8) % 8, cell[ids] // 64
+        assert np.all(cx // 4 + 2 * (cy // 2 + 4 * (cz // 2)) == k)
+    assert off_b[-1] == cfg.N
+
+
+def test_bad_bucket_sizes_are_rejected():
+    cfg = cfg_of(2, "f64", 10, (8, 8))
+    wl = W.make_workload(cfg)
+    g = O.grid_of(cfg)
+    for bad in [(0, 1), (9, 1), (1, -2)]:
+        with pytest.raises(Exception):
+            O.sort_buckets(g, wl.x, wl.v, wl.w, bad)
