@@ -166,6 +166,35 @@ int pic_step(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t 
              double dt, double qm, int do_sort, void *ws, size_t ws_bytes, void *stream);
 
 /*
+ * Buckets of several cells.  "Particles are sorted into buckets ... a bucket [is] one or more
+ * grid cells" (section 3.2); the paper's experiment is the sweep over the number of buckets
+ * (Fig. 9, 396-402 Fig. 14).  A bucket is a box of bucket[c] cells per dimension (1 <= bucket[c] <=
+ * n[c]; the last bucket of a dimension is smaller when bucket[c] does not divide n[c]); there are
+ * nb[c] = ceil(n[c] / bucket[c]) of them per dimension, ordered x fastest like the paper's bins ("ibin = bin %
+ * nsplitx; jbin = bin / nsplitx", App. B):
+ *     key_i = b_x + nb_x*(b_y + nb_y*b_z),  b_c = floor(cell_c / bucket[c]),  cell_c the clamped cell index of pic_sort.
+ * bucket is a HOST array of 3 ints (entries c >= dim ignored).  bucket = (1,1,1) gives exactly pic_sort / pic_step(PIC_SORT).
+ *
+ * pic_bucket_count: B = prod nb[c] (host computation).
+ * pic_sort_buckets: the stable counting sort of pic_sort with this key.  Particles of one bucket become contiguous and
+ *   keep their source order inside it (R7; the paper leaves it arbitrary).  bucket_offsets[B+1] is IN/OUT exactly like
+ *   pic_sort's cell_offsets (an optional order hint on entry; offsets of the buckets on return).  Workspace:
+ *   pic_workspace_bytes() of the grid.
+ * pic_step_buckets: sort by bucket, then the same deposit + gather + accel + push pass over the particles in bucket
+ *   order; rho, out as in pic_step.  The pass walks runs of equal CELL key; inside a bucket of several cells the order
+ *   is the source order, so runs are short and particles alone in their run go the threads-on-particles way
+ *   (setrho 3.3.4): the result is exact for every bucket size, the time grows with it (the sweep is in
+ *   profiles/ and DESIGN.md).
+ */
+int pic_bucket_count(const pic_grid_t *grid, const int32_t bucket[3] /* host */, int64_t *count /* host, out */);
+int pic_sort_buckets(const pic_grid_t *grid, const int32_t bucket[3] /* host */, const pic_particles_t *in,
+                     pic_particles_t *out, int32_t *perm, int32_t *bucket_offsets, void *ws, size_t ws_bytes,
+                     void *stream);
+int pic_step_buckets(const pic_grid_t *grid, const int32_t bucket[3] /* host */, const pic_particles_t *in,
+                     pic_particles_t *out, int32_t *perm, int32_t *bucket_offsets, void *rho,
+                     const void *const E[3], double dt, double qm, void *ws, size_t ws_bytes, void *stream);
+
+/*
  * pic_step_host -- the same step on HOST buffers: copies `in`, E to the device, runs pic_step,
  * copies out, perm, cell_offsets, rho back and synchronises.  All pointers (including those
  * inside in/out) are host pointers; dev_ws is a DEVICE scratch buffer of at least

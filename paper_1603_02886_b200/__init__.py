@@ -22,6 +22,7 @@ PIC_SORT, PIC_SORT_CHAINED = 1, 3
 
 EXPORTS = ("pic_workspace_bytes", "pic_sort", "pic_deposit", "pic_push", "pic_step",
            "pic_step_host_bytes", "pic_step_host", "pic_step_fields_host_bytes", "pic_step_fields_host",
+           "pic_bucket_count", "pic_sort_buckets", "pic_step_buckets",
            "pic_last_launch_count", "pic_set_phase_events",
            "pic_strerror")
 PHASES = ("begin", "keys", "scan", "radix", "reorder", "deposit", "push")
@@ -75,6 +76,10 @@ def lib():
         L.pic_step_host.argtypes = [G, P, P, vp, vp, vp, E3, dbl, dbl, ci, vp, sz, vp]
         L.pic_step_fields_host_bytes.argtypes = [G, i64, ctypes.POINTER(sz)]
         L.pic_step_fields_host.argtypes = [G, P, P, vp, vp, vp, E3, dbl, dbl, ci, vp, sz, vp]
+        B3 = ctypes.POINTER(ctypes.c_int32)
+        L.pic_bucket_count.argtypes = [G, B3, ctypes.POINTER(i64)]
+        L.pic_sort_buckets.argtypes = [G, B3, P, P, vp, vp, vp, sz, vp]
+        L.pic_step_buckets.argtypes = [G, B3, P, P, vp, vp, vp, E3, dbl, dbl, vp, sz, vp]
         L.pic_last_launch_count.argtypes = []
         L.pic_set_phase_events.argtypes = [ctypes.POINTER(ctypes.c_void_p), ci]
         L.pic_strerror.argtypes = [ci]
@@ -211,6 +216,44 @@ def pic_sort(g: Grid, x_in, v_in, w_in, x_out, v_out, w_out, perm, cell_offsets,
     pi, po = _particles(g, x_in, v_in, w_in, n), _particles(g, x_out, v_out, w_out, n)
     _check(lib().pic_sort(ctypes.byref(cg), ctypes.byref(pi), ctypes.byref(po), _ptr(perm), _ptr(cell_offsets),
                           _ptr(ws), ws.numel() * ws.element_size(), _stream(stream)), "pic_sort")
+
+
+def _bucket3(g: Grid, bucket):
+    b = [int(v) for v in bucket]
+    if len(b) != g.dim:
+        raise PicError("bucket must have one entry per dimension")
+    return (ctypes.c_int32 * 3)(*(b + [1] * (3 - g.dim)))
+
+
+def pic_bucket_count(g: Grid, bucket) -> int:
+    """Number of buckets of bucket[c] cells per dimension on this grid (host computation)."""
+    cg, out = g.c(), ctypes.c_int64(0)
+    _check(lib().pic_bucket_count(ctypes.byref(cg), _bucket3(g, bucket), ctypes.byref(out)), "pic_bucket_count")
+    return int(out.value)
+
+
+def pic_sort_buckets(g: Grid, bucket, x_in, v_in, w_in, x_out, v_out, w_out, perm, bucket_offsets, ws, stream=None):
+    """Stable sort by BUCKET key (boxes of bucket[c] cells): out_a[j] = in_a[perm[j]]; bucket_offsets[B+1]."""
+    n = w_in.numel()
+    _dev_check(g, list(x_in) + list(v_in) + [w_in] + list(x_out) + list(v_out) + [w_out], n)
+    cg = g.c()
+    pi, po = _particles(g, x_in, v_in, w_in, n), _particles(g, x_out, v_out, w_out, n)
+    _check(lib().pic_sort_buckets(ctypes.byref(cg), _bucket3(g, bucket), ctypes.byref(pi), ctypes.byref(po), _ptr(perm),
+                                  _ptr(bucket_offsets), _ptr(ws), ws.numel() * ws.element_size(), _stream(stream)),
+           "pic_sort_buckets")
+
+
+def pic_step_buckets(g: Grid, bucket, x_in, v_in, w_in, x_out, v_out, w_out, perm, bucket_offsets, rho, E, dt: float,
+                     qm: float, ws, stream=None):
+    """sort by bucket -> deposit at x(t) -> accel -> push; out = particles in bucket order at t+1."""
+    n = w_in.numel()
+    _dev_check(g, list(x_in) + list(v_in) + [w_in] + list(x_out) + list(v_out) + [w_out], n)
+    _dev_check(g, list(E) + [rho], g.cells)
+    cg = g.c()
+    pi, po = _particles(g, x_in, v_in, w_in, n), _particles(g, x_out, v_out, w_out, n)
+    _check(lib().pic_step_buckets(ctypes.byref(cg), _bucket3(g, bucket), ctypes.byref(pi), ctypes.byref(po), _ptr(perm),
+                                  _ptr(bucket_offsets), _ptr(rho), _field(g, E), dt, qm, _ptr(ws),
+                                  ws.numel() * ws.element_size(), _stream(stream)), "pic_step_buckets")
 
 
 def pic_deposit(g: Grid, x, w, rho, order_state=PIC_ORDER_UNSORTED, cell_offsets=None, ws=None, stream=None):

@@ -84,6 +84,14 @@ static bool aliases(const pic_grid_t& g, const pic_particles_t& a, const pic_par
     return false;
 }
 
+static int check_bucket(const pic_grid_t& g, const int32_t* bucket)
+{
+    if (!bucket) return PIC_ERR_INVALID_ARG;
+    for (int c = 0; c < g.dim; ++c)
+        if (bucket[c] < 1 || bucket[c] > g.n[c]) return PIC_ERR_INVALID_ARG;
+    return PIC_OK;
+}
+
 static int check_field(const pic_grid_t& g, const void* const E[3])
 {
     if (!E) return PIC_ERR_INVALID_ARG;
@@ -235,6 +243,64 @@ int pic_step(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
     if ((rc = launch_deposit(*grid, o, PIC_ORDER_UNSORTED, nullptr, rho, sws.racc, st)) != PIC_OK) return rc;
     mark_phase(PIC_PHASE_DEPOSIT, st);
     rc = launch_push(*grid, o, PIC_ORDER_UNSORTED, nullptr, E, dt, qm, st);
+    mark_phase(PIC_PHASE_PUSH, st);
+    return rc;
+}
+
+// ---- buckets of several cells (NEXT-2) -------------------------------------------------------
+int pic_bucket_count(const pic_grid_t* grid, const int32_t bucket[3], int64_t* count)
+{
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if ((rc = check_bucket(*grid, bucket)) != PIC_OK) return rc;
+    if (!count) return PIC_ERR_INVALID_ARG;
+    int64_t B = 1;
+    for (int c = 0; c < grid->dim; ++c) B *= (grid->n[c] + bucket[c] - 1) / bucket[c];
+    *count = B;
+    return PIC_OK;
+}
+
+int pic_sort_buckets(const pic_grid_t* grid, const int32_t bucket[3], const pic_particles_t* in, pic_particles_t* out,
+                     int32_t* perm, int32_t* bucket_offsets, void* ws, size_t ws_bytes, void* stream)
+{
+    g_launches = 0;
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if ((rc = check_bucket(*grid, bucket)) != PIC_OK) return rc;
+    if ((rc = check_particles(*grid, in, true, true)) != PIC_OK) return rc;
+    if ((rc = check_particles(*grid, out, true, true, in->n)) != PIC_OK) return rc;
+    if ((in->n > 0 && !aligned16(perm)) || !aligned16(bucket_offsets) || !aligned16(ws)) return PIC_ERR_INVALID_ARG;
+    if (in->n > 0 && aliases(*grid, *in, *out, in->n)) return PIC_ERR_INVALID_ARG;
+    SortWs sws;
+    if ((rc = carve_sort_ws(*grid, in->n, ws, ws_bytes, sws, bucket)) != PIC_OK) return rc;
+    pic_particles_t o = *out;
+    o.n = in->n;
+    return launch_sort(*grid, *in, o, perm, bucket_offsets, sws, true, false, (cudaStream_t)stream);
+}
+
+int pic_step_buckets(const pic_grid_t* grid, const int32_t bucket[3], const pic_particles_t* in, pic_particles_t* out,
+                     int32_t* perm, int32_t* bucket_offsets, void* rho, const void* const E[3], double dt, double qm,
+                     void* ws, size_t ws_bytes, void* stream)
+{
+    g_launches = 0;
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if ((rc = check_bucket(*grid, bucket)) != PIC_OK) return rc;
+    if ((rc = check_particles(*grid, in, true, true)) != PIC_OK) return rc;
+    if ((rc = check_particles(*grid, out, true, true, in->n)) != PIC_OK) return rc;
+    if ((rc = check_field(*grid, E)) != PIC_OK) return rc;
+    if (!aligned16(rho) || !aligned16(ws)) return PIC_ERR_INVALID_ARG;
+    if ((in->n > 0 && !aligned16(perm)) || !aligned16(bucket_offsets)) return PIC_ERR_INVALID_ARG;
+    if (in->n > 0 && aliases(*grid, *in, *out, in->n)) return PIC_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    SortWs sws;
+    if ((rc = carve_sort_ws(*grid, in->n, ws, ws_bytes, sws, bucket)) != PIC_OK) return rc;
+    pic_particles_t o = *out;
+    o.n = in->n;
+    if ((rc = launch_sort(*grid, *in, o, perm, bucket_offsets, sws, false, false, st)) != PIC_OK) return rc;
+    bool unit = true;                            // one cell per bucket: this is pic_step(PIC_SORT)
+    for (int c = 0; c < grid->dim; ++c) unit = unit && bucket[c] == 1;
+    rc = launch_fused(*grid, *in, o, perm, sws, rho, E, dt, qm, st, unit);
     mark_phase(PIC_PHASE_PUSH, st);
     return rc;
 }

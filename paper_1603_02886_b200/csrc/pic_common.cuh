@@ -25,10 +25,12 @@ struct GridP {
     T inv_vol;       // 1 / prod h
     int hmul;        // 1: every h is a power of two, x*inv_h == x/h bit for bit
     double Ld[3];    // box length in double (advance_wrap)
+    int bk[3];       // cells per bucket and dimension (sort key of pic_sort_buckets; 1 = one cell per bucket)
+    int nbk[3];      // buckets per dimension = ceil(n / bk)
 };
 
 template <typename T>
-inline GridP<T> make_gridp(const pic_grid_t& g)
+inline GridP<T> make_gridp(const pic_grid_t& g, const int32_t* bucket = nullptr)
 {
     GridP<T> p;
     double vol = 1.0;
@@ -43,6 +45,8 @@ inline GridP<T> make_gridp(const pic_grid_t& g)
         p.L[c] = (T)L;
         p.Ld[c] = L;
         p.inv_L[c] = (T)(1.0 / L);
+        p.bk[c] = (on && bucket) ? bucket[c] : 1;
+        p.nbk[c] = (p.n[c] + p.bk[c] - 1) / p.bk[c];
         if (on) {
             vol *= h;
             int e;
@@ -88,6 +92,22 @@ template <typename T>
 __device__ __forceinline__ int cell_index(T t, int n)
 {
     return max(0, min(floor_to_int(t), n - 1));
+}
+
+// Sort key of a particle from its clamped cell indices.  BK = false: the cell key, x fastest (a1,
+// PAPER.md:489-490).  BK = true: the key of its BUCKET, a box of bk[c] cells per dimension, buckets x fastest
+// ("a bucket ... one or more grid cells"; "ibin = bin % nsplitx; jbin = bin / nsplitx",
+// PAPER.md:487-490): key = b_x + nb_x (b_y + nb_y b_z), b_c = floor(cell_c / bk_c).
+template <typename T, int D, bool BK>
+__device__ __forceinline__ int sort_key(const GridP<T>& g, const int (&cell)[3])
+{
+    int k = 0, mul = 1;
+#pragma unroll
+    for (int c = 0; c < D; ++c) {
+        k += mul * (BK ? cell[c] / g.bk[c] : cell[c]);
+        mul *= BK ? g.nbk[c] : g.n[c];
+    }
+    return k;
 }
 
 // One-dimensional stencil of degree P: first (unfolded) node and the P+1 weights.
@@ -230,10 +250,13 @@ struct SortWs {
     size_t zero_bytes;
     int passes, bits_per_pass, key_bits;
     int64_t radix_tiles, scan_tiles, cls_tiles, stage_tiles;
+    int64_t nkeys;           // number of sort keys: cells, or buckets
+    const int32_t* bucket;   // host: cells per bucket and dimension, or NULL (one cell per bucket)
 };
 
 size_t sort_ws_bytes(const pic_grid_t& g, int64_t n);
-int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, SortWs& out);
+// bucket != NULL (host, bucket[c] cells per dimension): the sort key is the bucket, not the cell (pic_sort_buckets)
+int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, SortWs& out, const int32_t* bucket = nullptr);
 
 // reorder = false: only perm and cell_offsets are produced (out is not written).  chained: the caller says that
 // `in` is the unmodified output of the previous pic_step on this workspace (checked on the device against the
@@ -250,8 +273,10 @@ int launch_push(const pic_grid_t& g, pic_particles_t& p, int order_state, const 
 // the same pass).  With perm, *ws.gate (written by the sort: 1 = most particles move) chooses on the device
 // between that one pass and reorder-then-in-place; without perm, *ws.stray_count is zeroed here.  Lone
 // particles go through ws.stray_list to a threads-on-particles kernel.
+// cell_sorted = false (with perm): perm groups the particles by bucket only (pic_step_buckets); nothing is emitted.
 int launch_fused(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
-                 const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st);
+                 const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st,
+                 bool cell_sorted = true);
 // out_a[j] = in_a[perm[j]] for every attribute; runs only if *gate == want (gate may be NULL)
 int launch_reorder(const pic_grid_t& g, const pic_particles_t& in, const pic_particles_t& out, const int32_t* perm,
                    const uint32_t* gate, uint32_t want, cudaStream_t st);

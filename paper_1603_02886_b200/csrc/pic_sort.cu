@@ -197,7 +197,7 @@ static_assert(kClsTile <= (1 << 12), "13-bit fields of BlockHist");
 static_assert(kClsTile % kStageTile == 0 && kStageTile % (32 * kClsIPT) == 0, "staging tiles are whole warps of a classify block");
 
 // One warp's 32*kClsIPT positions.  CHECK = false: all of them are below n (no bounds tests).
-template <typename T, int D, bool CHECK>
+template <typename T, int D, bool CHECK, bool BK>
 __device__ __forceinline__ void classify_warp(const PartP<T>& p, const GridP<T>& g, int n, int wbase, unsigned lane, bool hint_ok,
                                               const int32_t* __restrict__ old_off, const BlockHist& hist,
                                               uint32_t* __restrict__ pkey, uint32_t (&key)[kClsIPT], uint32_t (&bal)[kClsIPT],
@@ -214,13 +214,10 @@ __device__ __forceinline__ void classify_warp(const PartP<T>& p, const GridP<T>&
     }
 #pragma unroll
     for (int r = 0; r < kClsIPT; ++r) {
-        int k = 0, mul = 1;
+        int cell[3] = {0, 0, 0};
 #pragma unroll
-        for (int c = 0; c < D; ++c) {
-            T t = grid_coord(xs[c][r], g.h[c], g.inv_h[c], g.hmul);
-            k += mul * cell_index(t, g.n[c]);
-            mul *= g.n[c];
-        }
+        for (int c = 0; c < D; ++c) cell[c] = cell_index(grid_coord(xs[c][r], g.h[c], g.inv_h[c], g.hmul), g.n[c]);
+        const int k = sort_key<T, D, BK>(g, cell);
         key[r] = (!CHECK || i0 + r * 32 < n) ? (uint32_t)k : 0xFFFFFFFFu;
         if (!CHECK || i0 + r * 32 < n) pkey[i0 + r * 32] = (uint32_t)k;
     }
@@ -282,7 +279,7 @@ __device__ __forceinline__ void classify_warp(const PartP<T>& p, const GridP<T>&
     }
 }
 
-template <typename T, int D>
+template <typename T, int D, bool BK>
 #ifndef PIC_CLS_MINB
 #define PIC_CLS_MINB 4
 #endif
@@ -307,9 +304,9 @@ k_classify(PartP<T> p, GridP<T> g, int n, const int32_t* __restrict__ old_off, i
     uint32_t key[kClsIPT], bal[kClsIPT];
     uint32_t mover_bits, lo_bits;
     if (wbase + 32 * kClsIPT <= n)
-        classify_warp<T, D, false>(p, g, n, wbase, lane, hint_ok, old_off, hist, pkey, key, bal, mover_bits, lo_bits);
+        classify_warp<T, D, false, BK>(p, g, n, wbase, lane, hint_ok, old_off, hist, pkey, key, bal, mover_bits, lo_bits);
     else
-        classify_warp<T, D, true>(p, g, n, wbase, lane, hint_ok, old_off, hist, pkey, key, bal, mover_bits, lo_bits);
+        classify_warp<T, D, true, BK>(p, g, n, wbase, lane, hint_ok, old_off, hist, pkey, key, bal, mover_bits, lo_bits);
 
     // movers before each word of this warp, warp total
     uint32_t wpre[kClsIPT], wtotal = 0;
@@ -792,10 +789,29 @@ static SortLayout sort_layout(const pic_grid_t& g, int64_t n)
 
 size_t sort_ws_bytes(const pic_grid_t& g, int64_t n) { return sort_layout(g, n).total; }
 
-int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, SortWs& o)
+// number of sort keys: cells, or buckets of bucket[c] cells per dimension
+int64_t sort_keys_of(const pic_grid_t& g, const int32_t* bucket)
+{
+    int64_t K = 1;
+    for (int c = 0; c < g.dim; ++c) K *= bucket ? (g.n[c] + bucket[c] - 1) / bucket[c] : g.n[c];
+    return K;
+}
+
+int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, SortWs& o, const int32_t* bucket)
 {
     SortLayout L = sort_layout(g, n);
     if (ws_bytes < L.total) return PIC_ERR_WORKSPACE;
+    if (bucket) {                                        // fewer keys than cells: the arrays are large enough; fewer radix bits
+        const int64_t K = sort_keys_of(g, bucket);
+        int b = 1;
+        while (((int64_t)1 << b) < K) ++b;
+        L.key_bits = b;
+        L.passes = (b + kRadixBits - 1) / kRadixBits;
+        L.bits = (b + L.passes - 1) / L.passes;
+        L.scan_tiles = (K + kScanTile - 1) / kScanTile;
+    }
+    o.nkeys = sort_keys_of(g, bucket);
+    o.bucket = bucket;
     char* b = (char*)ws;
     o.keys[0] = (uint32_t*)(b + L.keys0);
     o.keys[1] = (uint32_t*)(b + L.keys1);
@@ -870,7 +886,7 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
                           const SortWs& ws, bool chained, cudaStream_t st)
 {
     const int64_t n = in.n;
-    const int C = (int)cells_of(g);
+    const int C = (int)ws.nkeys;                      // cells, or buckets (pic_sort_buckets)
     mark_phase(PIC_PHASE_BEGIN, st);
     PIC_CUDA_OK(cudaMemsetAsync(ws.zero_begin, 0, ws.zero_bytes, st));
     // the hint: cell_offsets as found on entry -- or, in a chain, what the previous step left in the workspace
@@ -883,8 +899,9 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
         k_zero_hist<<<sm_count() * 4, 256, 0, st>>>((uint4*)ws.hist_begin, ws.hist_bytes / 16, ws.counters);
         k_chain_counts<<<(unsigned)((C + 255) / 256), 256, 0, st>>>(ws.old_off, ws.emit.cell_out, ws.emit.mover_in, ws.cell_count,
                                                                     ws.mover_count, ws.mover_lo, C, ws.counters);
-        k_classify<T, D><<<(unsigned)ws.cls_tiles, kClsThreads, 0, st>>>(
-            make_partp<T>(in), make_gridp<T>(g), (int)n, ws.old_off, ws.cell_count, ws.mover_count, ws.mover_lo, ws.keys[1],
+        auto classify = ws.bucket ? k_classify<T, D, true> : k_classify<T, D, false>;
+        classify<<<(unsigned)ws.cls_tiles, kClsThreads, 0, st>>>(
+            make_partp<T>(in), make_gridp<T>(g, ws.bucket), (int)n, ws.old_off, ws.cell_count, ws.mover_count, ws.mover_lo, ws.keys[1],
             ws.idx[1], ws.mask, ws.mprefix, ws.tile_count, ws.pkey, ws.counters);
         k_scan_cells<<<(unsigned)((ws.stage_tiles + kScanTile - 1) / kScanTile), kScanThreads, 0, st>>>(
             ws.tile_count, ws.tile_base, (int)ws.stage_tiles, ws.cls_status, ws.counters + kCtrCls, nullptr, 0, 0);

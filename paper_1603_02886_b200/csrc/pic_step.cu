@@ -9,14 +9,27 @@ namespace pic {
 
 template <typename T, int D, int P>
 static int fused_impl(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
-                      const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st)
+                      const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st, bool cell_sorted)
 {
     int64_t C = 1;
     for (int c = 0; c < g.dim; ++c) C *= g.n[c];
     double* racc = sizeof(T) == 8 ? (double*)rho : ws.racc;
     PIC_CUDA_OK(cudaMemsetAsync(racc, 0, sizeof(double) * (size_t)C, st));
     int rc;
-    if (perm) {
+    if (perm && !cell_sorted) {
+        // perm groups the particles by BUCKET (pic_step_buckets): inside a bucket of several cells they keep their
+        // source order, so a run of equal cell key is short and most particles are alone in theirs.  The same pass;
+        // lone particles are set aside for k_strays (threads on particles, setrho 3.3.4), the others
+        // go run by run.  Nothing is emitted (the next sort's key is not the cell key).
+        PIC_CUDA_OK(cudaMemsetAsync(ws.chain_sig, 0, sizeof(ChainSig), st));
+        PIC_CUDA_OK(cudaMemsetAsync(ws.stray_count, 0, sizeof(uint32_t), st));
+        rc = launch_runs<T, D, P, kModeBoth, true>(g, src, p, perm, E, racc, dt, qm, st, ws.gate, 0u, ws.stray_list, ws.stray_count);
+        if (rc != PIC_OK) return rc;
+        if ((rc = launch_reorder(g, src, p, perm, ws.gate, 1u, st)) != PIC_OK) return rc;
+        rc = launch_runs<T, D, P, kModeBoth, false>(g, p, p, nullptr, E, racc, dt, qm, st, ws.gate, 1u, ws.stray_list, ws.stray_count);
+        if (rc != PIC_OK) return rc;
+        if ((rc = launch_strays<T, D, P, kModeBoth>(g, p, E, racc, dt, qm, ws.stray_list, ws.stray_count, sm_count(), st)) != PIC_OK) return rc;
+    } else if (perm) {
         // steady state: ONE pass through perm.  Most particles moving (first step, garbage hint): the scattered
         // gather is done by the high-occupancy reorder kernel first and the pass runs in place.  *ws.gate, written
         // by the sort, selects on the device: the kernels of the other arm return at once.  Either way the pass
@@ -46,23 +59,23 @@ static int fused_impl(const pic_grid_t& g, const pic_particles_t& src, pic_parti
 
 template <typename T, int D>
 static int fused_order(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
-                       const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st)
+                       const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st, bool cell_sorted)
 {
     switch (g.order) {
-    case 1: return fused_impl<T, D, 1>(g, src, p, perm, ws, rho, E, dt, qm, st);
-    case 2: return fused_impl<T, D, 2>(g, src, p, perm, ws, rho, E, dt, qm, st);
-    default: return fused_impl<T, D, 3>(g, src, p, perm, ws, rho, E, dt, qm, st);
+    case 1: return fused_impl<T, D, 1>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted);
+    case 2: return fused_impl<T, D, 2>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted);
+    default: return fused_impl<T, D, 3>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted);
     }
 }
 
 int launch_fused(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
-                 const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st)
+                 const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st, bool cell_sorted)
 {
     if (g.dtype == PIC_F32)
-        return g.dim == 2 ? fused_order<float, 2>(g, src, p, perm, ws, rho, E, dt, qm, st)
-                          : fused_order<float, 3>(g, src, p, perm, ws, rho, E, dt, qm, st);
-    return g.dim == 2 ? fused_order<double, 2>(g, src, p, perm, ws, rho, E, dt, qm, st)
-                      : fused_order<double, 3>(g, src, p, perm, ws, rho, E, dt, qm, st);
+        return g.dim == 2 ? fused_order<float, 2>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted)
+                          : fused_order<float, 3>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted);
+    return g.dim == 2 ? fused_order<double, 2>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted)
+                      : fused_order<double, 3>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted);
 }
 
 }  // namespace pic
