@@ -482,15 +482,13 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
                 const bool live = u + grp < end;
                 const int r = live ? u + grp : end - 1;
                 const uint32_t rp = a_rec + (uint32_t)(r * RECS) * B;
-                T wxv[S], wyv[RPL];
-                lds<T, S>(rp, wxv);
+                T wyv[RPL];
+                Pk<T> wx2[S2];
+                lds_pairs<S2>(rp, wx2);
                 lds<T, RPL>(rp + (uint32_t)(S + jj0) * B, wyv);
                 const T wzv = (D == 3) ? lds1<T>(rp + (uint32_t)(2 * S + kk) * B) : (T)1;
                 T qv = (T)0;
                 if constexpr (DEP) { qv = lds1<T>(a_q + (uint32_t)r * B); qv = live ? qv : (T)0; }
-                Pk<T> wx2[S2];
-#pragma unroll
-                for (int i = 0; i < S2; ++i) wx2[i] = pk_make(wxv[2 * i], wxv[2 * i + 1]);
                 Pk<T> sum[PUSH ? D : 1];
                 const Pk<T> q2 = pk_make(qv, qv);
                 bool first = true;
@@ -563,19 +561,21 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
             }
             const bool mover = valid && nk != key;
             const unsigned bal = __ballot_sync(FULL, mover);
-            if (valid) em.pkey[jl + b0] = (uint32_t)nk;
+            const uint32_t slot = (uint32_t)j0 + (uint32_t)(b0 + lane);   // N < 2^30: 32-bit slot numbers
+            if (valid) em.pkey[slot] = (uint32_t)nk;
             if (mover) {
                 const uint32_t at = (uint32_t)j0 + emitted + (uint32_t)__popc(bal & ((1u << lane) - 1u));
                 em.stage_key[at] = (uint32_t)nk;
-                em.stage_idx[at] = (uint32_t)(jl + b0);
+                em.stage_idx[at] = slot;
                 // histograms: one particle fewer in the present cell, one mover more in the next one (the second
                 // word counts those that come from below); the sort puts count = old count - out + in together
                 atomicAdd(&em.cell_out[key], 1);
                 atomicAdd(&em.mover_in[nk], (nk > key) ? 0x100000001ull : 1ull);
             }
             if (lane == 0) {
-                em.mask[(j0 + b0) >> 5] = bal;
-                em.mprefix[(j0 + b0) >> 5] = emitted;
+                const uint32_t word = ((uint32_t)j0 + (uint32_t)b0) >> 5;
+                em.mask[word] = bal;
+                em.mprefix[word] = emitted;
             }
             emitted += (uint32_t)__popc(bal);
         }

@@ -183,6 +183,25 @@ __device__ __forceinline__ void lds(uint32_t a, T (&o)[N])
         for (int i = 0; i < N; ++i) asm volatile("ld.shared.f64 %0, [%1];" : "=d"(o[i]) : "r"(a + 8 * i));
     }
 }
+// S consecutive elements at byte address a (aligned to 16) as S/2 packed pairs: the fp32 pairs arrive in
+// 64-bit registers, so no move packs them
+template <int S2>
+__device__ __forceinline__ void lds_pairs(uint32_t a, Pk<float> (&o)[S2])
+{
+    if constexpr (S2 == 2) {
+        asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(o[0].r), "=l"(o[1].r) : "r"(a));
+    } else {
+#pragma unroll
+        for (int i = 0; i < S2; ++i) asm volatile("ld.shared.b64 %0, [%1];" : "=l"(o[i].r) : "r"(a + 8 * i));
+    }
+}
+template <int S2>
+__device__ __forceinline__ void lds_pairs(uint32_t a, Pk<double> (&o)[S2])
+{
+#pragma unroll
+    for (int i = 0; i < S2; ++i)
+        asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(o[i].lo), "=d"(o[i].hi) : "r"(a + 16 * i));
+}
 template <typename T>
 __device__ __forceinline__ T lds1(uint32_t a)
 {

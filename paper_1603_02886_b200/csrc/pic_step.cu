@@ -25,7 +25,7 @@ static int fused_impl(const pic_grid_t& g, const pic_particles_t& src, pic_parti
         PIC_CUDA_OK(cudaMemsetAsync(ws.stray_count, 0, sizeof(uint32_t), st));
         rc = launch_runs<T, D, P, kModeBoth, true>(g, src, p, perm, E, racc, dt, qm, st, ws.gate, 0u, ws.stray_list, ws.stray_count);
         if (rc != PIC_OK) return rc;
-        if ((rc = launch_reorder(g, src, p, perm, ws.gate, 1u, st)) != PIC_OK) return rc;
+        if ((rc = launch_reorder_records(g, src, p, perm, ws.rec_scratch, ws.gate, 1u, st)) != PIC_OK) return rc;
         rc = launch_runs<T, D, P, kModeBoth, false>(g, p, p, nullptr, E, racc, dt, qm, st, ws.gate, 1u, ws.stray_list, ws.stray_count);
         if (rc != PIC_OK) return rc;
         if ((rc = launch_strays<T, D, P, kModeBoth>(g, p, E, racc, dt, qm, ws.stray_list, ws.stray_count, sm_count(), st)) != PIC_OK) return rc;
@@ -37,7 +37,7 @@ static int fused_impl(const pic_grid_t& g, const pic_particles_t& src, pic_parti
         PIC_CUDA_OK(cudaMemsetAsync(ws.emit_begin, 0, ws.emit_bytes, st));
         rc = launch_runs<T, D, P, kModeBoth, true>(g, src, p, perm, E, racc, dt, qm, st, ws.gate, 0u, nullptr, nullptr, &ws.emit);
         if (rc != PIC_OK) return rc;
-        if ((rc = launch_reorder(g, src, p, perm, ws.gate, 1u, st)) != PIC_OK) return rc;
+        if ((rc = launch_reorder_records(g, src, p, perm, ws.rec_scratch, ws.gate, 1u, st)) != PIC_OK) return rc;
         rc = launch_runs<T, D, P, kModeBoth, false>(g, p, p, nullptr, E, racc, dt, qm, st, ws.gate, 1u, nullptr, nullptr, &ws.emit);
         if (rc != PIC_OK) return rc;
         if (p.n > 0 && (rc = launch_chain_commit(g, p, ws, st)) != PIC_OK) return rc;
