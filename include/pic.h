@@ -124,6 +124,22 @@ int pic_deposit(const pic_grid_t *grid, const pic_particles_t *p, int order_stat
                 const int32_t *cell_offsets, void *rho, void *ws, size_t ws_bytes, void *stream);
 
 /*
+ * pic_deposit_nodes -- the same rho by the paper's COLLISION-FREE algorithm, "threads on splines" (setrho_splines,
+ * PAPER.md:202-204 section 3.3.1 and Fig. 6; Fortran of App. B): the threads are
+ * associated with the grid nodes, each node adds up the spline values of the particles of the cells around it, nothing
+ * is written twice, no atomics.  Cost as the paper counts it, (Nx+d)(Ny+d)(Nz+d) Np/Nbuckets, with one cell per bucket.
+ * p must be sorted by cell and cell_offsets[C+1] must be the offsets of that order (pic_sort's output).
+ * The additions of a node happen in a FIXED order -- ascending position in the sorted array -- in double, every
+ * operation rounded on its own: rho is bitwise reproducible from run to run, and it IS the particle-order double sum
+ * of the definition (rounded once to float for fp32 grids).  pic_deposit gives the same numbers to rounding, faster.
+ * If cell_offsets does not describe the order of p (checked on the device) the call still returns the correct rho,
+ * computed by pic_deposit's any-order kernel, without the reproducibility.
+ * ws: at least pic_workspace_bytes(), for both dtypes.  rho[C] is overwritten.
+ */
+int pic_deposit_nodes(const pic_grid_t *grid, const pic_particles_t *p, const int32_t *cell_offsets,
+                      void *rho, void *ws, size_t ws_bytes, void *stream);
+
+/*
  * pic_push -- field gather + accel + push in one pass (rows a6-a7; PAPER.md:82-83 steps iii-iv,
  * 86, 88; models PAPER.md:312, 316):
  *   E_i = sum_j E[j] * prod_c W_p(x_ic/h_c - j_c)   (same splines as the deposit)

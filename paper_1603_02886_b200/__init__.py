@@ -22,7 +22,7 @@ PIC_SORT, PIC_SORT_CHAINED = 1, 3
 
 EXPORTS = ("pic_workspace_bytes", "pic_sort", "pic_deposit", "pic_push", "pic_step",
            "pic_step_host_bytes", "pic_step_host", "pic_step_fields_host_bytes", "pic_step_fields_host",
-           "pic_bucket_count", "pic_sort_buckets", "pic_step_buckets",
+           "pic_bucket_count", "pic_sort_buckets", "pic_step_buckets", "pic_deposit_nodes",
            "pic_last_launch_count", "pic_set_phase_events",
            "pic_strerror")
 PHASES = ("begin", "keys", "scan", "radix", "reorder", "deposit", "push")
@@ -80,6 +80,7 @@ def lib():
         L.pic_bucket_count.argtypes = [G, B3, ctypes.POINTER(i64)]
         L.pic_sort_buckets.argtypes = [G, B3, P, P, vp, vp, vp, sz, vp]
         L.pic_step_buckets.argtypes = [G, B3, P, P, vp, vp, vp, E3, dbl, dbl, vp, sz, vp]
+        L.pic_deposit_nodes.argtypes = [G, P, vp, vp, vp, sz, vp]
         L.pic_last_launch_count.argtypes = []
         L.pic_set_phase_events.argtypes = [ctypes.POINTER(ctypes.c_void_p), ci]
         L.pic_strerror.argtypes = [ci]
@@ -266,6 +267,18 @@ def pic_deposit(g: Grid, x, w, rho, order_state=PIC_ORDER_UNSORTED, cell_offsets
     wsb = ws.numel() * ws.element_size() if ws is not None else 0
     _check(lib().pic_deposit(ctypes.byref(cg), ctypes.byref(p), order_state, _ptr(cell_offsets), _ptr(rho),
                              _ptr(ws), wsb, _stream(stream)), "pic_deposit")
+
+
+def pic_deposit_nodes(g: Grid, x, w, rho, cell_offsets, ws, stream=None):
+    """rho[C] by the collision-free threads-on-nodes algorithm: fixed order of additions, bitwise reproducible.
+    x, w sorted by cell; cell_offsets from pic_sort."""
+    n = w.numel()
+    _dev_check(g, list(x) + [w], n)
+    _dev_check(g, [rho], g.cells)
+    cg = g.c()
+    p = _particles(g, x, None, w, n)
+    _check(lib().pic_deposit_nodes(ctypes.byref(cg), ctypes.byref(p), _ptr(cell_offsets), _ptr(rho), _ptr(ws),
+                                   ws.numel() * ws.element_size(), _stream(stream)), "pic_deposit_nodes")
 
 
 def pic_push(g: Grid, x, v, E, dt: float, qm: float, order_state=PIC_ORDER_UNSORTED, cell_offsets=None,

@@ -278,6 +278,9 @@ int launch_push(const pic_grid_t& g, pic_particles_t& p, int order_state, const 
 int launch_fused(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
                  const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st,
                  bool cell_sorted = true);
+// the collision-free deposit with a fixed order of additions (pic_nodes.cu); p sorted by cell as cell_offsets says
+int launch_deposit_nodes(const pic_grid_t& g, const pic_particles_t& p, const int32_t* cell_offsets, void* rho,
+                         const SortWs& ws, cudaStream_t st);
 // out_a[j] = in_a[perm[j]] for every attribute; runs only if *gate == want (gate may be NULL)
 int launch_reorder(const pic_grid_t& g, const pic_particles_t& in, const pic_particles_t& out, const int32_t* perm,
                    const uint32_t* gate, uint32_t want, cudaStream_t st);
