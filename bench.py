@@ -200,11 +200,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg3")
     ap.add_argument("--particles", type=int, default=0, help="override N (debug; invalidates the headline)")
+    ap.add_argument("--grid", default="", help="override the grid, e.g. 512,256 (the paper's Fig. 9 / Fig. 14 shape; not the headline)")
     ap.add_argument("--sort-every", type=int, default=0)
     ap.add_argument("--ppc", type=int, default=0, help="config 5: particles per cell")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cold", action="store_true")
+    ap.add_argument("--bucket", default="", help="cells per bucket, e.g. 2,2,2: the sort steps are pic_step_buckets "
+                    "(the paper's bucket-size sweep, PAPER.md:336-350; not the headline)")
+    ap.add_argument("--deposit-compare", action="store_true",
+                    help="also time pic_deposit (sorted / never sorted) and pic_deposit_nodes on this workload")
     ap.add_argument("--ref-particles", type=int, default=2_000_000)
     ap.add_argument("--cpu-particles", type=int, default=30_000_000)
     args = ap.parse_args()
@@ -218,6 +223,8 @@ def main():
     cfg = W.CONFIGS[args.config]
     if args.config == "cfg5":
         cfg = W.cfg5(args.ppc or 128, args.sort_every or 1)
+    if args.grid:
+        cfg = cfg.scaled(cfg.N, n=tuple(int(k) for k in args.grid.split(",")))
     if args.particles:
         cfg = cfg.scaled(args.particles)
     if args.sort_every:
@@ -249,7 +256,8 @@ def main():
     stt.step(tiny.dt, tiny.qm, False)
     torch.cuda.synchronize()
     del stt, wt
-    st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, device=dev)
+    bucket = tuple(int(b) for b in args.bucket.split(",")) if args.bucket else None
+    st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, device=dev, bucket=bucket)
     torch.cuda.synchronize()
 
     def barrier():
@@ -384,8 +392,8 @@ def main():
     # config 5 asks for the deposit with and without sorting (the paper's sorted vs unsorted columns,
     # PAPER.md:392-394): pic_deposit on the current sorted order, and on the never-sorted initial order
     deposit_compare = None
-    if args.config == "cfg5" and world == 1:
-        deposit_compare = run_deposit_compare(B, torch, cfg, g, wl, st, dev)
+    if (args.config == "cfg5" or args.deposit_compare) and world == 1 and bucket is None:
+        deposit_compare = run_deposit_compare(B, torch, cfg, g, wl, st, dev, nodes=args.deposit_compare)
 
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
@@ -399,6 +407,9 @@ def main():
             "step_roofline": {"bytes_per_particle_step": bytes_step, "achieved": step_ach, "peak": peak,
                               "frac": step_ach / peak, "frac_of_8TBps_nominal": step_ach / 8000.0, "unit": "GB/s"},
             "phase_ms": phase_ms, "first_step_ms": first_ms, "cold": cold}
+    if bucket is not None:
+        line["config"]["bucket"] = list(bucket)
+        line["config"]["workload"] += ", buckets of %s cells (pic_step_buckets)" % "x".join(map(str, bucket))
     if deposit_compare:
         line["deposit_ms"] = deposit_compare
     if e2e_resident:
@@ -474,7 +485,7 @@ def run_e2e_resident(B, torch, cfg, g, wl, st, dev, K, world, dist):
             "api": "pic_step_fields_host (particles resident on the device; E in, rho out, pinned host buffers)"}
 
 
-def run_deposit_compare(B, torch, cfg, g, wl, st, dev, reps=5):
+def run_deposit_compare(B, torch, cfg, g, wl, st, dev, reps=5, nodes=False):
     """ms per pic_deposit call: particles sorted by cell (per-cell kernel) against the same workload never
     sorted (threads on particles with global atomics, setrho 3.3.4)."""
     def timed(f):
@@ -494,11 +505,19 @@ def run_deposit_compare(B, torch, cfg, g, wl, st, dev, reps=5):
     ws_ = torch.empty_like(a["w"])
     B.pic_sort(g, a["x"], a["v"], a["w"], xs, vs, ws_, st.perm, st.cell_offsets, st.ws)
     t_sorted = timed(lambda: B.pic_deposit(g, xs, ws_, st.rho, B.PIC_ORDER_SORTED, st.cell_offsets, st.ws))
+    t_nodes = None
+    if nodes:      # the collision-free, bitwise reproducible alternative (threads on splines)
+        reps, keep = 2, reps
+        t_nodes = timed(lambda: B.pic_deposit_nodes(g, xs, ws_, st.rho, st.cell_offsets, st.ws))
+        reps = keep
     del vs
     x0 = [torch.from_numpy(np.ascontiguousarray(t)).to(dev) for t in wl.x]
     w0 = torch.from_numpy(np.ascontiguousarray(wl.w)).to(dev)
     t_unsorted = timed(lambda: B.pic_deposit(g, x0, w0, st.rho, B.PIC_ORDER_UNSORTED, None, st.ws))
-    return {"sorted": t_sorted, "never_sorted": t_unsorted, "unit": "ms per deposit of all particles"}
+    out = {"sorted": t_sorted, "never_sorted": t_unsorted, "unit": "ms per deposit of all particles"}
+    if t_nodes is not None:
+        out["nodes_deterministic"] = t_nodes
+    return out
 
 
 def run_cpu_baseline(cfg, sample):

@@ -281,3 +281,57 @@ def step(g: Grid, x, v, w, E, dt: float, qm: float, do_sort: bool = True, cell_o
                              _ptrs(E), ctypes.c_double(dt), ctypes.c_double(qm),
                              ctypes.c_int(1 if do_sort else 0)))
     return dict(x=xo, v=vo, w=wo, perm=perm, cell_offsets=off, rho=rho)
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-4: the field solve, step ii of the loop -- "field_solver(): -Laplace(phi) = rho"
+# (section 3; "we solve Poisson's equation for computing the field potential phi"),
+# periodic boundary conditions.  The paper leaves the step out ("Step ii involving field_solver is
+# not considered"), so everything beyond the equation is a reading (R21-R23):
+#   R21  E = -grad(phi) (electrostatics; "the forces on each particle from the electric potential")
+#   R22  the mean of rho is dropped (a periodic box is solvable only for zero net charge: uniform neutralising
+#        background); phi has zero mean
+#   R23  spectral discretisation on the node grid: with rho^ = DFT(rho) and wave numbers
+#        kappa_c(m) = 2 pi mt / L_c, mt = m for m <= n/2, m - n above,
+#        phi^ = rho^ / sum_c kappa_c^2,   E_c^ = -i kappa'_c phi^,
+#        kappa' = kappa except kappa' = 0 at the Nyquist index m = n/2 of an even n (the derivative of that
+#        mode of a real grid function is not a real grid function).
+# Plain numpy, float64; np.fft.fftn / ifftn are the library primitive that serves as the step.  Pinned in
+# tests/test_oracle_field.py against the analytic single-mode solution, a brute-force O(C^2) Fourier sum on
+# tiny grids, the finite-difference Gauss law on smooth fields and the cold-plasma oscillation frequency.
+def field_solve(g: Grid, rho):
+    """(phi, [E_c]) on the node grid, x fastest, float64."""
+    shape = tuple(reversed(g.n[: g.dim]))                        # C order: z, y, x
+    r = np.asarray(rho, np.float64).reshape(shape)
+    rh = np.fft.fftn(r)
+    kap, kapd = [], []
+    for c in range(g.dim):
+        n, L = g.n[c], g.n[c] * g.h[c]
+        m = np.arange(n)
+        mt = np.where(m <= n // 2, m, m - n).astype(np.float64)
+        k = 2.0 * np.pi * mt / L
+        kd = k.copy()
+        if n % 2 == 0:
+            kd[n // 2] = 0.0
+        ax = [1] * g.dim
+        ax[g.dim - 1 - c] = n
+        kap.append(k.reshape(ax))
+        kapd.append(kd.reshape(ax))
+    k2 = sum(k * k for k in kap)
+    k2[(0,) * g.dim] = 1.0
+    ph = rh / k2
+    ph[(0,) * g.dim] = 0.0
+    phi = np.real(np.fft.ifftn(ph)).reshape(-1)
+    E = [np.real(np.fft.ifftn(-1j * kapd[c] * ph)).reshape(-1) for c in range(g.dim)]
+    return phi, E
+
+
+def step_selfconsistent(g: Grid, x, v, w, dt: float, qm: float):
+    """One step of the closed loop i-iv: sort -> setrho -> field_solver -> accel -> push.
+    E is stored in the grid's dtype before the push, as the CUDA path stores it.  -> dict like step() plus E, phi."""
+    xs, vs, ws, perm, off = sort(g, x, v, w)
+    rho = deposit(g, xs, ws)
+    phi, E = field_solve(g, rho)
+    Es = [e.astype(g.np_dtype) for e in E]
+    xo, vo = push(g, xs, vs, Es, dt, qm)
+    return dict(x=xo, v=vo, w=ws, perm=perm, cell_offsets=off, rho=rho, E=Es, phi=phi)

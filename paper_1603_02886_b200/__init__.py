@@ -342,9 +342,12 @@ def pic_step_fields_host(g: Grid, x_in, v_in, w_in, x_out, v_out, w_out, perm, c
 class Stepper:
     """Device-resident particle state with ping-pong buffers: the usual way to run many steps."""
 
-    def __init__(self, g: Grid, x, v, w, E, device="cuda"):
+    def __init__(self, g: Grid, x, v, w, E, device="cuda", bucket=None):
+        """bucket: cells per bucket and dimension -> the sort steps are pic_step_buckets (cell_offsets then holds the
+        BUCKET offsets); None: pic_step."""
         import torch
         self.g, self.n = g, int(w.shape[0])
+        self.bucket = None if bucket is None else tuple(int(b) for b in bucket)
         dev = torch.device(device)
         up = lambda a: torch.as_tensor(a).to(dev).contiguous()
         self.cur = dict(x=[up(a) for a in x], v=[up(a) for a in v], w=up(w))
@@ -374,7 +377,11 @@ class Stepper:
         particle arrays and nothing else writes them between steps, which is what that flag states (the library
         checks the rest, so the first step and a step after reset() or an unsorted step fall back by themselves)."""
         a, b = self.cur, self.nxt
-        if do_sort:
+        if do_sort and self.bucket is not None:
+            pic_step_buckets(self.g, self.bucket, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], self.perm,
+                             self.cell_offsets, self.rho, self.E, dt, qm, self.ws, stream)
+            self.cur, self.nxt = b, a
+        elif do_sort:
             pic_step(self.g, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], self.perm, self.cell_offsets,
                      self.rho, self.E, dt, qm, PIC_SORT_CHAINED if (chained and self._chain_ok) else PIC_SORT,
                      self.ws, stream)

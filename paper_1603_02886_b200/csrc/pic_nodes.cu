@@ -38,9 +38,21 @@ __global__ void __launch_bounds__(256) k_offsets_check(const int32_t* __restrict
     if (b) *bad = 1u;
 }
 
+// num / 6 correctly rounded, without the division routine: q = RN(num * RN(1/6)) is within an ulp of the quotient,
+// r = num - 6 q is exact in one fused operation, and RN(q + r * RN(1/6)) is then the correctly rounded quotient
+// (Markstein's correction step; 6 is exactly representable and RN(1/6) is the correctly rounded reciprocal).
+__device__ __forceinline__ double div6_rn(double num)
+{
+    const double y = 1.0 / 6.0;                            // RN(1/6), folded at compile time
+    const double q = __dmul_rn(num, y);
+    const double r = __fma_rn(-6.0, q, num);
+    return __fma_rn(r, y, q);
+}
+
 // 1-D weight of a particle on the node with stencil index a (0..P), every operation rounded on its own, in the
 // order of the definition's polynomial forms (R1): p = 1 (1 - xi, xi); p = 2 with d = xi - (nearest node - i0);
-// p = 3 ((1-xi)^3, 3 xi^3 - 6 xi^2 + 4, -3 xi^3 + 3 xi^2 + 3 xi + 1, xi^3) / 6.
+// p = 3 ((1-xi)^3, 3 xi^3 - 6 xi^2 + 4, -3 xi^3 + 3 xi^2 + 3 xi + 1, xi^3) / 6.  Branch-free: the lanes of a warp are
+// neighbouring nodes and hold different a.
 template <int P>
 __device__ __forceinline__ bool node_weight(double xi, int i0, int jn, int n, double& w)
 {
@@ -56,34 +68,24 @@ __device__ __forceinline__ bool node_weight(double xi, int i0, int jn, int n, do
         first = i0 - 1;
     }
     int a = jn - first;                                  // first in [-2, n]: one fold either way
-    if (a < 0) a += n;
-    if (a >= n) a -= n;
-    if (a > P) return false;                             // the particle's stencil does not reach this node
+    a = a < 0 ? a + n : a;
+    a = a >= n ? a - n : a;
     if constexpr (P == 1) {
         w = a == 0 ? __dsub_rn(1.0, xi) : xi;
     } else if constexpr (P == 2) {
-        if (a == 1) {
-            w = __dsub_rn(0.75, __dmul_rn(d, d));
-        } else {
-            const double s = a == 0 ? __dsub_rn(0.5, d) : __dadd_rn(0.5, d);
-            w = __dmul_rn(__dmul_rn(0.5, s), s);
-        }
+        const double s = a == 0 ? __dsub_rn(0.5, d) : __dadd_rn(0.5, d);
+        const double side = __dmul_rn(__dmul_rn(0.5, s), s), mid = __dsub_rn(0.75, __dmul_rn(d, d));
+        w = a == 1 ? mid : side;
     } else {
         const double x2 = __dmul_rn(xi, xi), x3 = __dmul_rn(x2, xi);
-        double num;
-        if (a == 0) {
-            const double om = __dsub_rn(1.0, xi);
-            num = __dmul_rn(__dmul_rn(om, om), om);
-        } else if (a == 1) {
-            num = __dadd_rn(__dsub_rn(__dmul_rn(3.0, x3), __dmul_rn(6.0, x2)), 4.0);
-        } else if (a == 2) {
-            num = __dadd_rn(__dadd_rn(__dadd_rn(__dmul_rn(-3.0, x3), __dmul_rn(3.0, x2)), __dmul_rn(3.0, xi)), 1.0);
-        } else {
-            num = x3;
-        }
-        w = __ddiv_rn(num, 6.0);
+        const double om = __dsub_rn(1.0, xi);
+        const double n0 = __dmul_rn(__dmul_rn(om, om), om);
+        const double n1 = __dadd_rn(__dsub_rn(__dmul_rn(3.0, x3), __dmul_rn(6.0, x2)), 4.0);
+        const double n2 = __dadd_rn(__dadd_rn(__dadd_rn(__dmul_rn(-3.0, x3), __dmul_rn(3.0, x2)), __dmul_rn(3.0, xi)), 1.0);
+        const double num = a == 0 ? n0 : (a == 1 ? n1 : (a == 2 ? n2 : x3));
+        w = div6_rn(num);
     }
-    return true;
+    return a <= P;                                       // else the particle's stencil does not reach this node
 }
 
 // contribution of particle i to node jn[]; cc[] = the cell the particle must be in (else *wrong)
@@ -108,27 +110,29 @@ __device__ __forceinline__ bool node_contribution(const PartP<T>& p, const GridP
     return true;
 }
 
-// the cells of one dimension whose particles can reach node j: j-1, j (p = 1) or j-2 .. j+1 (p = 2, 3), folded,
-// ascending and without repeats (a small grid folds two of them onto each other)
+// the cells of one dimension whose particles can reach node j: j-1, j (p = 1) or j-2 .. j+1 (p = 2, 3), folded into
+// [0, n), in ASCENDING order and without repeats: cell number q of m = min(count, n).  A fold happens at one end
+// at most: the cells folded down from beyond n-1 come first, those folded up from below 0 last.
 template <int P>
-__device__ __forceinline__ int node_cells(int j, int n, int (&cell)[4])
-{
-    constexpr int lo = (P == 1) ? -1 : -2, cnt = (P == 1) ? 2 : 4;
-    int m = 0;
-    for (int k = 0; k < cnt; ++k) {
-        const int u = fold(j + lo + k, n);
-        bool seen = false;
-        for (int q = 0; q < m; ++q) seen = seen || cell[q] == u;
-        if (!seen) cell[m++] = u;
+struct NodeCells {
+    int m, hi, lw, base, n;
+    __device__ __forceinline__ NodeCells(int j, int n_) : n(n_)
+    {
+        constexpr int lo = (P == 1) ? -1 : -2, cnt = (P == 1) ? 2 : 4;
+        if (n_ < cnt) {                                   // a grid smaller than the reach: every cell, once
+            m = n_; hi = 0; lw = 0; base = 0;
+        } else {
+            m = cnt;
+            hi = max(0, j + lo + cnt - n_);
+            lw = max(0, -(j + lo));
+            base = max(j + lo, 0);
+        }
     }
-    for (int a = 1; a < m; ++a) {                          // insertion sort of at most 4 values
-        const int v = cell[a];
-        int b = a;
-        while (b > 0 && cell[b - 1] > v) { cell[b] = cell[b - 1]; --b; }
-        cell[b] = v;
+    __device__ __forceinline__ int cell(int q) const
+    {
+        return q < hi ? q : (q < m - lw ? base + (q - hi) : n - lw + (q - (m - lw)));
     }
-    return m;
-}
+};
 
 template <typename T, int D, int P>
 __global__ void __launch_bounds__(128) k_deposit_nodes(PartP<T> p, GridP<T> g, const int32_t* __restrict__ off, int64_t C,
@@ -142,15 +146,14 @@ __global__ void __launch_bounds__(128) k_deposit_nodes(PartP<T> p, GridP<T> g, c
     jn[0] = (int)(node % g.n[0]);
     jn[1] = (int)((node / g.n[0]) % g.n[1]);
     jn[2] = (D == 3) ? (int)(node / ((int64_t)g.n[0] * g.n[1])) : 0;
-    int cx[4], cy[4], cz[4] = {0, 0, 0, 0};
-    const int mx = node_cells<P>(jn[0], g.n[0], cx), my = node_cells<P>(jn[1], g.n[1], cy);
-    const int mz = (D == 3) ? node_cells<P>(jn[2], g.n[2], cz) : 1;
+    const NodeCells<P> ncx(jn[0], g.n[0]), ncy(jn[1], g.n[1]), ncz(jn[2], (D == 3) ? g.n[2] : 1);
+    const int mx = ncx.m, my = ncy.m, mz = (D == 3) ? ncz.m : 1;
     // how many particles sit around this node?
     int64_t visits = 0;
     for (int a = 0; a < mz; ++a)
         for (int b = 0; b < my; ++b)
             for (int c = 0; c < mx; ++c) {
-                const int64_t cell = cx[c] + (int64_t)g.n[0] * (cy[b] + (int64_t)g.n[1] * cz[a]);
+                const int64_t cell = ncx.cell(c) + (int64_t)g.n[0] * (ncy.cell(b) + (int64_t)g.n[1] * ((D == 3) ? ncz.cell(a) : 0));
                 visits += off[cell + 1] - off[cell];
             }
     if (visits > kDenseVisits) {                           // a warp takes it (k_deposit_nodes_dense)
@@ -162,7 +165,7 @@ __global__ void __launch_bounds__(128) k_deposit_nodes(PartP<T> p, GridP<T> g, c
     for (int a = 0; a < mz; ++a)                           // cells in ascending key = ascending position of their particles
         for (int b = 0; b < my; ++b)
             for (int c = 0; c < mx; ++c) {
-                const int cc[3] = {cx[c], cy[b], cz[a]};
+                const int cc[3] = {ncx.cell(c), ncy.cell(b), (D == 3) ? ncz.cell(a) : 0};
                 const int64_t cell = cc[0] + (int64_t)g.n[0] * (cc[1] + (int64_t)g.n[1] * cc[2]);
                 const int64_t end = off[cell + 1];
                 for (int64_t i = off[cell]; i < end; ++i) {
@@ -191,15 +194,14 @@ __global__ void __launch_bounds__(128) k_deposit_nodes_dense(PartP<T> p, GridP<T
         jn[0] = (int)(node % g.n[0]);
         jn[1] = (int)((node / g.n[0]) % g.n[1]);
         jn[2] = (D == 3) ? (int)(node / ((int64_t)g.n[0] * g.n[1])) : 0;
-        int cx[4], cy[4], cz[4] = {0, 0, 0, 0};
-        const int mx = node_cells<P>(jn[0], g.n[0], cx), my = node_cells<P>(jn[1], g.n[1], cy);
-        const int mz = (D == 3) ? node_cells<P>(jn[2], g.n[2], cz) : 1;
+        const NodeCells<P> ncx(jn[0], g.n[0]), ncy(jn[1], g.n[1]), ncz(jn[2], (D == 3) ? g.n[2] : 1);
+        const int mx = ncx.m, my = ncy.m, mz = (D == 3) ? ncz.m : 1;
         double acc = 0.0;
         bool wrong = false;
         for (int a = 0; a < mz; ++a)
             for (int b = 0; b < my; ++b)
                 for (int c = 0; c < mx; ++c) {
-                    const int cc[3] = {cx[c], cy[b], cz[a]};
+                    const int cc[3] = {ncx.cell(c), ncy.cell(b), (D == 3) ? ncz.cell(a) : 0};
                     const int64_t cell = cc[0] + (int64_t)g.n[0] * (cc[1] + (int64_t)g.n[1] * cc[2]);
                     const int64_t end = off[cell + 1];
                     for (int64_t i0 = off[cell]; i0 < end; i0 += 32) {
