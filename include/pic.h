@@ -211,6 +211,31 @@ int pic_step_buckets(const pic_grid_t *grid, const int32_t bucket[3] /* host */,
                      const void *const E[3], double dt, double qm, void *ws, size_t ws_bytes, void *stream);
 
 /*
+ * The field solve and the closed loop.  Step ii of the paper's loop, "field_solver(): -Laplace(phi) =
+ * rho" (section 3; "we solve Poisson's equation for computing the field potential phi"), with
+ * periodic boundary conditions.  The paper leaves the step out ("not considered"); beyond the
+ * equation everything is a reading (R21-R23): E = -grad(phi); the mean of rho is dropped (neutralising
+ * background) and phi has zero mean; spectral discretisation on the node grid: with rho^ = DFT(rho) and
+ * kappa_c(m) = 2 pi mt / L_c (mt = m for m <= n/2, m - n above), phi^ = rho^ / sum_c kappa_c^2 and E_c^ = -i kappa'_c phi^,
+ * kappa' = kappa except 0 at the Nyquist index of an even n.
+ *
+ * pic_field_solve: rho[C] -> E[c][C] for c < dim and, if phi != NULL, phi[C]; all of the grid's dtype, x fastest; the
+ *   arithmetic is double whatever the dtype.  Hand-written transforms (radix-2 for power-of-two n[c], the plain DFT sum
+ *   otherwise); n[c] <= 4096 else PIC_ERR_UNSUPPORTED.  ws: pic_field_solve_bytes().
+ * pic_step_selfconsistent: one step of the closed loop i-iv: sort by cell (cell_offsets: in/out hint as in
+ *   pic_sort), rho = deposit at x(t) (the reorder happens in the same pass), E = field_solve(rho) written to the
+ *   caller's E[c], then v += qm dt E(x), x += dt v on the sorted particles.  out, perm, cell_offsets, rho as in pic_step.
+ *   ws: pic_step_selfconsistent_bytes().
+ */
+int pic_field_solve_bytes(const pic_grid_t *grid, size_t *bytes /* host, out */);
+int pic_field_solve(const pic_grid_t *grid, const void *rho, void *const E[3], void *phi /* may be NULL */,
+                    void *ws, size_t ws_bytes, void *stream);
+int pic_step_selfconsistent_bytes(const pic_grid_t *grid, int64_t n, size_t *bytes /* host, out */);
+int pic_step_selfconsistent(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t *out,
+                            int32_t *perm, int32_t *cell_offsets, void *rho, void *const E[3],
+                            double dt, double qm, void *ws, size_t ws_bytes, void *stream);
+
+/*
  * pic_step_host -- the same step on HOST buffers: copies `in`, E to the device, runs pic_step,
  * copies out, perm, cell_offsets, rho back and synchronises.  All pointers (including those
  * inside in/out) are host pointers; dev_ws is a DEVICE scratch buffer of at least

@@ -23,6 +23,7 @@ PIC_SORT, PIC_SORT_CHAINED = 1, 3
 EXPORTS = ("pic_workspace_bytes", "pic_sort", "pic_deposit", "pic_push", "pic_step",
            "pic_step_host_bytes", "pic_step_host", "pic_step_fields_host_bytes", "pic_step_fields_host",
            "pic_bucket_count", "pic_sort_buckets", "pic_step_buckets", "pic_deposit_nodes",
+           "pic_field_solve_bytes", "pic_field_solve", "pic_step_selfconsistent_bytes", "pic_step_selfconsistent",
            "pic_last_launch_count", "pic_set_phase_events",
            "pic_strerror")
 PHASES = ("begin", "keys", "scan", "radix", "reorder", "deposit", "push")
@@ -81,6 +82,10 @@ def lib():
         L.pic_sort_buckets.argtypes = [G, B3, P, P, vp, vp, vp, sz, vp]
         L.pic_step_buckets.argtypes = [G, B3, P, P, vp, vp, vp, E3, dbl, dbl, vp, sz, vp]
         L.pic_deposit_nodes.argtypes = [G, P, vp, vp, vp, sz, vp]
+        L.pic_field_solve_bytes.argtypes = [G, ctypes.POINTER(sz)]
+        L.pic_field_solve.argtypes = [G, vp, E3, vp, vp, sz, vp]
+        L.pic_step_selfconsistent_bytes.argtypes = [G, i64, ctypes.POINTER(sz)]
+        L.pic_step_selfconsistent.argtypes = [G, P, P, vp, vp, vp, E3, dbl, dbl, vp, sz, vp]
         L.pic_last_launch_count.argtypes = []
         L.pic_set_phase_events.argtypes = [ctypes.POINTER(ctypes.c_void_p), ci]
         L.pic_strerror.argtypes = [ci]
@@ -279,6 +284,39 @@ def pic_deposit_nodes(g: Grid, x, w, rho, cell_offsets, ws, stream=None):
     p = _particles(g, x, None, w, n)
     _check(lib().pic_deposit_nodes(ctypes.byref(cg), ctypes.byref(p), _ptr(cell_offsets), _ptr(rho), _ptr(ws),
                                    ws.numel() * ws.element_size(), _stream(stream)), "pic_deposit_nodes")
+
+
+def pic_field_solve_bytes(g: Grid) -> int:
+    cg, out = g.c(), ctypes.c_size_t(0)
+    _check(lib().pic_field_solve_bytes(ctypes.byref(cg), ctypes.byref(out)), "pic_field_solve_bytes")
+    return int(out.value)
+
+
+def pic_field_solve(g: Grid, rho, E, phi, ws, stream=None):
+    """Periodic Poisson solve: rho[C] -> E[c][C] (and phi[C] unless None); -Laplace(phi) = rho - mean, E = -grad(phi)."""
+    _dev_check(g, [rho] + list(E) + ([phi] if phi is not None else []), g.cells)
+    cg = g.c()
+    _check(lib().pic_field_solve(ctypes.byref(cg), _ptr(rho), _field(g, E), _ptr(phi), _ptr(ws),
+                                 ws.numel() * ws.element_size(), _stream(stream)), "pic_field_solve")
+
+
+def pic_step_selfconsistent_bytes(g: Grid, n: int) -> int:
+    cg, out = g.c(), ctypes.c_size_t(0)
+    _check(lib().pic_step_selfconsistent_bytes(ctypes.byref(cg), n, ctypes.byref(out)), "pic_step_selfconsistent_bytes")
+    return int(out.value)
+
+
+def pic_step_selfconsistent(g: Grid, x_in, v_in, w_in, x_out, v_out, w_out, perm, cell_offsets, rho, E, dt: float,
+                            qm: float, ws, stream=None):
+    """One step of the closed loop: sort -> deposit -> field solve (E is WRITTEN) -> accel -> push."""
+    n = w_in.numel()
+    _dev_check(g, list(x_in) + list(v_in) + [w_in] + list(x_out) + list(v_out) + [w_out], n)
+    _dev_check(g, list(E) + [rho], g.cells)
+    cg = g.c()
+    pi, po = _particles(g, x_in, v_in, w_in, n), _particles(g, x_out, v_out, w_out, n)
+    _check(lib().pic_step_selfconsistent(ctypes.byref(cg), ctypes.byref(pi), ctypes.byref(po), _ptr(perm),
+                                         _ptr(cell_offsets), _ptr(rho), _field(g, E), dt, qm, _ptr(ws),
+                                         ws.numel() * ws.element_size(), _stream(stream)), "pic_step_selfconsistent")
 
 
 def pic_push(g: Grid, x, v, E, dt: float, qm: float, order_state=PIC_ORDER_UNSORTED, cell_offsets=None,

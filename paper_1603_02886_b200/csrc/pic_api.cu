@@ -321,6 +321,64 @@ int pic_step_buckets(const pic_grid_t* grid, const int32_t bucket[3], const pic_
     return rc;
 }
 
+// ---- field solve and the closed loop (NEXT-4) -------------------------------------------------
+int pic_field_solve_bytes(const pic_grid_t* grid, size_t* bytes)
+{
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if (!bytes) return PIC_ERR_INVALID_ARG;
+    *bytes = field_ws_bytes(*grid);
+    return PIC_OK;
+}
+
+int pic_field_solve(const pic_grid_t* grid, const void* rho, void* const E[3], void* phi, void* ws, size_t ws_bytes, void* stream)
+{
+    g_launches = 0;
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if (!aligned16(rho) || !E || !aligned16(ws) || (phi && !aligned16(phi))) return PIC_ERR_INVALID_ARG;
+    for (int c = 0; c < grid->dim; ++c)
+        if (!aligned16(E[c])) return PIC_ERR_INVALID_ARG;
+    if (ws_bytes < field_ws_bytes(*grid)) return PIC_ERR_WORKSPACE;
+    return launch_field_solve(*grid, rho, E, phi, ws, (cudaStream_t)stream);
+}
+
+int pic_step_selfconsistent_bytes(const pic_grid_t* grid, int64_t n, size_t* bytes)
+{
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if (!bytes || n < 0 || n >= ((int64_t)1 << 30)) return PIC_ERR_INVALID_ARG;
+    *bytes = sort_ws_bytes(*grid, n) + field_ws_bytes(*grid);
+    return PIC_OK;
+}
+
+int pic_step_selfconsistent(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t* out, int32_t* perm,
+                            int32_t* cell_offsets, void* rho, void* const E[3], double dt, double qm, void* ws,
+                            size_t ws_bytes, void* stream)
+{
+    g_launches = 0;
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if ((rc = check_particles(*grid, in, true, true)) != PIC_OK) return rc;
+    if ((rc = check_particles(*grid, out, true, true, in->n)) != PIC_OK) return rc;
+    if (!E || !aligned16(rho) || !aligned16(ws)) return PIC_ERR_INVALID_ARG;
+    for (int c = 0; c < grid->dim; ++c)
+        if (!aligned16(E[c])) return PIC_ERR_INVALID_ARG;
+    if ((in->n > 0 && !aligned16(perm)) || !aligned16(cell_offsets)) return PIC_ERR_INVALID_ARG;
+    if (in->n > 0 && aliases(*grid, *in, *out, in->n)) return PIC_ERR_INVALID_ARG;
+    const size_t sb = sort_ws_bytes(*grid, in->n);
+    if (ws_bytes < sb + field_ws_bytes(*grid)) return PIC_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    SortWs sws;
+    if ((rc = carve_sort_ws(*grid, in->n, ws, sb, sws)) != PIC_OK) return rc;
+    pic_particles_t o = *out;
+    o.n = in->n;
+    if ((rc = launch_sort(*grid, *in, o, perm, cell_offsets, sws, false, false, st)) != PIC_OK) return rc;
+    rc = launch_selfconsistent(*grid, *in, o, perm, sws, rho, E, (char*)ws + sb, dt, qm, st);
+    mark_phase(PIC_PHASE_PUSH, st);
+    return rc;
+}
+
 // ---- host-buffer entry point: the end-to-end path bench.py times ---------------------------
 struct HostLayout {
     size_t in[7], out[7], perm, offsets, rho, E[3], ws, total, ws_bytes;

@@ -281,6 +281,12 @@ int launch_fused(const pic_grid_t& g, const pic_particles_t& src, pic_particles_
 // the collision-free deposit with a fixed order of additions (pic_nodes.cu); p sorted by cell as cell_offsets says
 int launch_deposit_nodes(const pic_grid_t& g, const pic_particles_t& p, const int32_t* cell_offsets, void* rho,
                          const SortWs& ws, cudaStream_t st);
+// periodic Poisson solve (pic_field.cu): rho -> E[c] (and phi if not NULL), all [C] of the grid's dtype; ws: field_ws_bytes
+size_t field_ws_bytes(const pic_grid_t& g);
+int launch_field_solve(const pic_grid_t& g, const void* rho, void* const E[3], void* phi, void* ws, cudaStream_t st);
+// the closed loop i-iv: deposit along perm (+ reorder into p), field solve, gather + accel + push in place
+int launch_selfconsistent(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
+                          const SortWs& ws, void* rho, void* const E[3], void* field_ws, double dt, double qm, cudaStream_t st);
 // out_a[j] = in_a[perm[j]] for every attribute; runs only if *gate == want (gate may be NULL)
 int launch_reorder(const pic_grid_t& g, const pic_particles_t& in, const pic_particles_t& out, const int32_t* perm,
                    const uint32_t* gate, uint32_t want, cudaStream_t st);

@@ -68,6 +68,52 @@ static int fused_order(const pic_grid_t& g, const pic_particles_t& src, pic_part
     }
 }
 
+// The closed loop (PAPER.md:79-84 steps i-iv with the field solve in): rho at x(t) while the
+// particles are reordered (one pass along perm), field_solver, then accel + push in place with the new field.
+template <typename T, int D, int P>
+static int selfconsistent_impl(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
+                               const SortWs& ws, void* rho, void* const E[3], void* field_ws, double dt, double qm, cudaStream_t st)
+{
+    int64_t C = 1;
+    for (int c = 0; c < g.dim; ++c) C *= g.n[c];
+    double* racc = sizeof(T) == 8 ? (double*)rho : ws.racc;
+    PIC_CUDA_OK(cudaMemsetAsync(racc, 0, sizeof(double) * (size_t)C, st));
+    PIC_CUDA_OK(cudaMemsetAsync(ws.chain_sig, 0, sizeof(ChainSig), st));       // nothing is emitted: no chain from here
+    int rc = launch_runs<T, D, P, kModeDeposit, true>(g, src, p, perm, nullptr, racc, 0.0, 0.0, st, ws.gate, 0u);
+    if (rc != PIC_OK) return rc;
+    if ((rc = launch_reorder_records(g, src, p, perm, ws.rec_scratch, ws.gate, 1u, st)) != PIC_OK) return rc;
+    if ((rc = launch_runs<T, D, P, kModeDeposit, false>(g, p, p, nullptr, nullptr, racc, 0.0, 0.0, st, ws.gate, 1u)) != PIC_OK) return rc;
+    if (sizeof(T) == 4) {
+        k_round_rho<T><<<(unsigned)((C + 255) / 256), 256, 0, st>>>(racc, (T*)rho, C);
+        count_launch();
+    }
+    mark_phase(PIC_PHASE_DEPOSIT, st);
+    if ((rc = launch_field_solve(g, rho, E, nullptr, field_ws, st)) != PIC_OK) return rc;
+    const void* Ec[3] = {E[0], E[1], E[2]};
+    return launch_runs<T, D, P, kModePush, false>(g, p, p, nullptr, Ec, nullptr, dt, qm, st);
+}
+
+template <typename T, int D>
+static int selfconsistent_order(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
+                                const SortWs& ws, void* rho, void* const E[3], void* field_ws, double dt, double qm, cudaStream_t st)
+{
+    switch (g.order) {
+    case 1: return selfconsistent_impl<T, D, 1>(g, src, p, perm, ws, rho, E, field_ws, dt, qm, st);
+    case 2: return selfconsistent_impl<T, D, 2>(g, src, p, perm, ws, rho, E, field_ws, dt, qm, st);
+    default: return selfconsistent_impl<T, D, 3>(g, src, p, perm, ws, rho, E, field_ws, dt, qm, st);
+    }
+}
+
+int launch_selfconsistent(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
+                          const SortWs& ws, void* rho, void* const E[3], void* field_ws, double dt, double qm, cudaStream_t st)
+{
+    if (g.dtype == PIC_F32)
+        return g.dim == 2 ? selfconsistent_order<float, 2>(g, src, p, perm, ws, rho, E, field_ws, dt, qm, st)
+                          : selfconsistent_order<float, 3>(g, src, p, perm, ws, rho, E, field_ws, dt, qm, st);
+    return g.dim == 2 ? selfconsistent_order<double, 2>(g, src, p, perm, ws, rho, E, field_ws, dt, qm, st)
+                      : selfconsistent_order<double, 3>(g, src, p, perm, ws, rho, E, field_ws, dt, qm, st);
+}
+
 int launch_fused(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
                  const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st, bool cell_sorted)
 {
