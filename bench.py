@@ -208,6 +208,8 @@ def main():
     ap.add_argument("--no-cold", action="store_true")
     ap.add_argument("--bucket", default="", help="cells per bucket, e.g. 2,2,2: the sort steps are pic_step_buckets "
                     "(the paper's bucket-size sweep, PAPER.md:336-350; not the headline)")
+    ap.add_argument("--closed-loop", action="store_true",
+                    help="the timed step is pic_step_selfconsistent: sort, deposit, Poisson solve, accel, push (not the headline)")
     ap.add_argument("--deposit-compare", action="store_true",
                     help="also time pic_deposit (sorted / never sorted) and pic_deposit_nodes on this workload")
     ap.add_argument("--ref-particles", type=int, default=2_000_000)
@@ -257,7 +259,9 @@ def main():
     torch.cuda.synchronize()
     del stt, wt
     bucket = tuple(int(b) for b in args.bucket.split(",")) if args.bucket else None
-    st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, device=dev, bucket=bucket)
+    if args.closed_loop:       # mean charge density one, so that the self-consistent field is of order one
+        wl.w = (wl.w * (cfg.cells / cfg.N)).astype(wl.w.dtype)
+    st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, device=dev, bucket=bucket, closed_loop=args.closed_loop)
     torch.cuda.synchronize()
 
     def barrier():
@@ -407,6 +411,9 @@ def main():
             "step_roofline": {"bytes_per_particle_step": bytes_step, "achieved": step_ach, "peak": peak,
                               "frac": step_ach / peak, "frac_of_8TBps_nominal": step_ach / 8000.0, "unit": "GB/s"},
             "phase_ms": phase_ms, "first_step_ms": first_ms, "cold": cold}
+    if args.closed_loop:
+        line["config"]["workload"] += ", closed loop with the periodic Poisson solve (pic_step_selfconsistent)"
+        line["config"]["closed_loop"] = True
     if bucket is not None:
         line["config"]["bucket"] = list(bucket)
         line["config"]["workload"] += ", buckets of %s cells (pic_step_buckets)" % "x".join(map(str, bucket))

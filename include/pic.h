@@ -168,12 +168,14 @@ int pic_push(const pic_grid_t *grid, pic_particles_t *p, int order_state,
  *   the two calls gives a wrong order.  In a chain the hint is the workspace's own copy of the previous
  *   offsets; cell_offsets is only written.
  * do_sort = 0: particles keep their order (out_a[j] = advanced in_a[j]; out may be the same arrays as
- * in); perm is not written and cell_offsets is not modified.  cell_offsets may be NULL (any-order
- * kernels) or the offsets of an EARLIER sort of these particles: they are then used to walk the
- * particles cell by cell, and a particle that has left its cell since is taken on its own
- * (threads-on-particles, setrho 3.3.4).  The result is exact whatever cell_offsets
- * holds: offsets that cannot be walked (checked on the device: off[0] = 0, off[C] = N, non-decreasing)
- * select the any-order kernels.  This is config 5's "sort every 4 / 16 steps" arm.
+ * in); perm is not written and cell_offsets is not modified.  cell_offsets NULL says "no order at all": the any-order
+ * kernels run (threads on particles, setrho 3.3.4).  cell_offsets non-NULL says "these particles
+ * were sorted some steps ago": the step kernel then walks runs of equal cell key, which it finds from the
+ * positions themselves (the array's contents are not read), and a particle that has drifted out of the run around
+ * it is taken on its own (threads on particles).  The result is exact whatever the order really is.
+ * This is config 5's "sort every 4 / 16 steps" arm.  On this hardware it is slower than
+ * sorting every step: a particle that has left its cell since the last sort pays (p+1)^d global reductions and
+ * uncoalesced field reads, a re-sort of the 15-25 % movers costs far less (numbers in DESIGN.md section 5.4).
  */
 #define PIC_SORT 1
 #define PIC_SORT_CHAINED 3

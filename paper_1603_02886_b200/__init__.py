@@ -380,9 +380,10 @@ def pic_step_fields_host(g: Grid, x_in, v_in, w_in, x_out, v_out, w_out, perm, c
 class Stepper:
     """Device-resident particle state with ping-pong buffers: the usual way to run many steps."""
 
-    def __init__(self, g: Grid, x, v, w, E, device="cuda", bucket=None):
+    def __init__(self, g: Grid, x, v, w, E, device="cuda", bucket=None, closed_loop=False):
         """bucket: cells per bucket and dimension -> the sort steps are pic_step_buckets (cell_offsets then holds the
-        BUCKET offsets); None: pic_step."""
+        BUCKET offsets); None: pic_step.  closed_loop: the sort steps are pic_step_selfconsistent (E is recomputed from
+        rho every step; the E given here only sizes the arrays)."""
         import torch
         self.g, self.n = g, int(w.shape[0])
         self.bucket = None if bucket is None else tuple(int(b) for b in bucket)
@@ -395,7 +396,9 @@ class Stepper:
         self.perm = torch.empty(max(self.n, 4), dtype=torch.int32, device=dev)
         self.cell_offsets = torch.zeros(g.cells + 4, dtype=torch.int32, device=dev)
         self.rho = torch.empty(g.cells, dtype=g.torch_dtype, device=dev)
-        self.ws = torch.empty(pic_workspace_bytes(g, self.n), dtype=torch.uint8, device=dev)
+        self.closed_loop = bool(closed_loop)
+        nbytes = pic_step_selfconsistent_bytes(g, self.n) if self.closed_loop else pic_workspace_bytes(g, self.n)
+        self.ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
         self.sorted_once = False
         self._chain_ok = False
 
@@ -415,7 +418,11 @@ class Stepper:
         particle arrays and nothing else writes them between steps, which is what that flag states (the library
         checks the rest, so the first step and a step after reset() or an unsorted step fall back by themselves)."""
         a, b = self.cur, self.nxt
-        if do_sort and self.bucket is not None:
+        if do_sort and self.closed_loop:
+            pic_step_selfconsistent(self.g, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], self.perm, self.cell_offsets,
+                                    self.rho, self.E, dt, qm, self.ws, stream)
+            self.cur, self.nxt = b, a
+        elif do_sort and self.bucket is not None:
             pic_step_buckets(self.g, self.bucket, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], self.perm,
                              self.cell_offsets, self.rho, self.E, dt, qm, self.ws, stream)
             self.cur, self.nxt = b, a
