@@ -208,6 +208,8 @@ def main():
     ap.add_argument("--no-cold", action="store_true")
     ap.add_argument("--bucket", default="", help="cells per bucket, e.g. 2,2,2: the sort steps are pic_step_buckets "
                     "(the paper's bucket-size sweep, PAPER.md:336-350; not the headline)")
+    ap.add_argument("--graph", action="store_true",
+                    help="replay the steps from CUDA graphs (small, launch-bound problems; no per-phase times)")
     ap.add_argument("--closed-loop", action="store_true",
                     help="the timed step is pic_step_selfconsistent: sort, deposit, Poisson solve, accel, push (not the headline)")
     ap.add_argument("--deposit-compare", action="store_true",
@@ -261,7 +263,7 @@ def main():
     bucket = tuple(int(b) for b in args.bucket.split(",")) if args.bucket else None
     if args.closed_loop:       # mean charge density one, so that the self-consistent field is of order one
         wl.w = (wl.w * (cfg.cells / cfg.N)).astype(wl.w.dtype)
-    st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, device=dev, bucket=bucket, closed_loop=args.closed_loop)
+    st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, device=dev, bucket=bucket, closed_loop=args.closed_loop, graph=args.graph)
     torch.cuda.synchronize()
 
     def barrier():
@@ -297,9 +299,10 @@ def main():
     t_begin.record()
     for k in range(K):
         do_sort = (step_no % cfg.sort_every == 0)
-        B.pic_set_phase_events(phase_ev[k])
+        if not args.graph:
+            B.pic_set_phase_events(phase_ev[k])
         st.step(cfg.dt, cfg.qm, do_sort=do_sort)
-        launches += B.pic_last_launch_count()
+        launches += (st.last_launches if (args.graph and do_sort and st.last_launches) else B.pic_last_launch_count())
         sorts += int(do_sort)
         step_no += 1
     t_end.record()
@@ -357,6 +360,24 @@ def main():
     bytes_step = ab["step"] if cfg.sort_every == 1 else (ab["step"] * sorts + ab["nosort_step"] * (K - sorts)) / K
     step_ach = bytes_step * cfg.N / (ms_step * 1e-3) / 1e9
 
+    # ---- the same steady-state steps replayed from CUDA graphs (no host launches inside the timed region)
+    graph_line = None
+    if not args.graph and cfg.sort_every == 1:
+        st.use_graph = True
+        for _ in range(4):                                   # captures one graph per ping-pong direction
+            st.step(cfg.dt, cfg.qm, do_sort=True)
+        barrier()
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record()
+        for _ in range(K):
+            st.step(cfg.dt, cfg.qm, do_sort=True)
+        g1.record()
+        barrier()
+        st.use_graph = False
+        gms = max_over_ranks(g0.elapsed_time(g1), dist if world > 1 else None, dev)
+        graph_line = {"ms_per_step": gms / K, "value": replica_throughput(cfg.N, world, K, gms), "unit": UNIT, "steps": K,
+                      "what": "the same steps replayed from two CUDA graphs (Stepper(graph=True)); the headline above is the plain launch path, whose per-phase events it needs"}
+
     # ---- the configuration as BASELINE.json words it: its own number of steps FROM THE SEEDED, UNSORTED state
     #      (the first step sorts every particle), one timed region, max over ranks
     cold = None
@@ -411,12 +432,16 @@ def main():
             "step_roofline": {"bytes_per_particle_step": bytes_step, "achieved": step_ach, "peak": peak,
                               "frac": step_ach / peak, "frac_of_8TBps_nominal": step_ach / 8000.0, "unit": "GB/s"},
             "phase_ms": phase_ms, "first_step_ms": first_ms, "cold": cold}
+    if args.graph:
+        line["config"]["cuda_graph"] = "sort steps replayed from CUDA graphs (one per ping-pong direction)"
     if args.closed_loop:
         line["config"]["workload"] += ", closed loop with the periodic Poisson solve (pic_step_selfconsistent)"
         line["config"]["closed_loop"] = True
     if bucket is not None:
         line["config"]["bucket"] = list(bucket)
         line["config"]["workload"] += ", buckets of %s cells (pic_step_buckets)" % "x".join(map(str, bucket))
+    if graph_line:
+        line["cuda_graph"] = graph_line
     if deposit_compare:
         line["deposit_ms"] = deposit_compare
     if e2e_resident:

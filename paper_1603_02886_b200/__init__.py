@@ -380,10 +380,13 @@ def pic_step_fields_host(g: Grid, x_in, v_in, w_in, x_out, v_out, w_out, perm, c
 class Stepper:
     """Device-resident particle state with ping-pong buffers: the usual way to run many steps."""
 
-    def __init__(self, g: Grid, x, v, w, E, device="cuda", bucket=None, closed_loop=False):
+    def __init__(self, g: Grid, x, v, w, E, device="cuda", bucket=None, closed_loop=False, graph=False):
         """bucket: cells per bucket and dimension -> the sort steps are pic_step_buckets (cell_offsets then holds the
         BUCKET offsets); None: pic_step.  closed_loop: the sort steps are pic_step_selfconsistent (E is recomputed from
-        rho every step; the E given here only sizes the arrays)."""
+        rho every step; the E given here only sizes the arrays).  graph: the sort steps are replayed from CUDA graphs
+        (one per direction of the ping-pong), which takes the 20-odd launches of a step off the host: for problems so
+        small that the step is launch bound.  Every choice inside a step (first or pre-ordered sort, chained or not)
+        is made on the device, so one captured step serves all of them."""
         import torch
         self.g, self.n = g, int(w.shape[0])
         self.bucket = None if bucket is None else tuple(int(b) for b in bucket)
@@ -397,6 +400,9 @@ class Stepper:
         self.cell_offsets = torch.zeros(g.cells + 4, dtype=torch.int32, device=dev)
         self.rho = torch.empty(g.cells, dtype=g.torch_dtype, device=dev)
         self.closed_loop = bool(closed_loop)
+        self.use_graph = bool(graph)
+        self._graphs = {}
+        self.last_launches = 0
         nbytes = pic_step_selfconsistent_bytes(g, self.n) if self.closed_loop else pic_workspace_bytes(g, self.n)
         self.ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
         self.sorted_once = False
@@ -418,14 +424,44 @@ class Stepper:
         particle arrays and nothing else writes them between steps, which is what that flag states (the library
         checks the rest, so the first step and a step after reset() or an unsorted step fall back by themselves)."""
         a, b = self.cur, self.nxt
+        if do_sort and self.use_graph and stream is None:
+            self._graph_step(dt, qm, chained)
+            return
+        self._enqueue(a, b, dt, qm, do_sort, stream, chained)
+
+    def _graph_step(self, dt, qm, chained):
+        """replay (capture on first use) the sort step from the current buffers into the other set"""
+        import torch
+        a, b = self.cur, self.nxt
+        self.last_launches = 0
+        if not self.sorted_once:                # the first step runs as it is (it also loads the kernels)
+            self._enqueue(a, b, dt, qm, True, None, chained)
+            return
+        key = (a["w"].data_ptr(), float(dt), float(qm), bool(chained and self._chain_ok))
+        if key not in self._graphs:
+            gr = torch.cuda.CUDAGraph()
+            state = (self.cur, self.nxt, self._chain_ok, self.sorted_once)
+            torch.cuda.synchronize()
+            with torch.cuda.graph(gr):
+                self._enqueue(a, b, dt, qm, True, None, chained)
+            self.cur, self.nxt, self._chain_ok, self.sorted_once = state      # capturing runs nothing
+            self._graphs[key] = (gr, pic_last_launch_count())
+        gr, self.last_launches = self._graphs[key]
+        gr.replay()
+        self.cur, self.nxt = b, a
+        self._chain_ok = not (self.closed_loop or self.bucket is not None)
+
+    def _enqueue(self, a, b, dt, qm, do_sort, stream, chained):
         if do_sort and self.closed_loop:
             pic_step_selfconsistent(self.g, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], self.perm, self.cell_offsets,
                                     self.rho, self.E, dt, qm, self.ws, stream)
             self.cur, self.nxt = b, a
+            self.sorted_once = True
         elif do_sort and self.bucket is not None:
             pic_step_buckets(self.g, self.bucket, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], self.perm,
                              self.cell_offsets, self.rho, self.E, dt, qm, self.ws, stream)
             self.cur, self.nxt = b, a
+            self.sorted_once = True
         elif do_sort:
             pic_step(self.g, a["x"], a["v"], a["w"], b["x"], b["v"], b["w"], self.perm, self.cell_offsets,
                      self.rho, self.E, dt, qm, PIC_SORT_CHAINED if (chained and self._chain_ok) else PIC_SORT,

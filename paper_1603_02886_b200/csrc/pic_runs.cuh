@@ -45,7 +45,7 @@ namespace pic {
 #define PIC_RUNS_MINW32 16      // resident warps per SM the fp32 kernels are compiled for
 #endif
 #ifndef PIC_RUNS_MINW64
-#define PIC_RUNS_MINW64 8
+#define PIC_RUNS_MINW64 10
 #endif
 #ifndef PIC_RUNS_WR
 #define PIC_RUNS_WR 2048        // slots per warp
@@ -73,14 +73,18 @@ struct RunsShape {
     static constexpr int NPL = (NODES + 31) / 32;                // stencil positions a lane fetches and flushes
     static constexpr int WR = PIC_RUNS_WR;
     static constexpr int RECW = D * S;                           // wx[S] wy[S] (wz[S])
-    static constexpr int REC4 = (RECW + 3) / 4;
-    static constexpr int RECS = 4 * (REC4 | 1);                  // odd number of 16-byte units: conflict-free rows
+    // strides of the per-particle rows in shared memory: an ODD number of 16-byte units, so that the 32 lanes of a
+    // 128-bit access (lane = particle) spread over all banks (fp64 rows of 96 and 192 bytes hit 4 and 2 of the 8
+    // 16-byte columns: half of that kernel's shared-memory wavefronts were bank conflicts)
+    static constexpr int EPU = 16 / (int)sizeof(T);              // elements per 16-byte unit
+    static constexpr int RECS = (((RECW + EPU - 1) / EPU) | 1) * EPU;      // weight record
+    static constexpr int PARTS = (((D * G + EPU - 1) / EPU) | 1) * EPU;    // partial fields of one particle: [D][G]
     static constexpr int kFlushEvery = sizeof(T) == 4 ? 128 * NG : (1 << 30);
     // shared memory of one warp, in elements of T
     static constexpr int oRec = 0;                               // [32][RECS] weight records of the batch
     static constexpr int oQ = oRec + 32 * RECS;                  // [32] w / prod h
-    static constexpr int oPart = oQ + 32;                        // [32][D][G] partial fields
-    static constexpr int oBuf = oPart + 32 * D * G;              // [NG][NODES] node sums / [D][NODES] field of a cell
+    static constexpr int oPart = oQ + 32;                        // [32][PARTS] partial fields
+    static constexpr int oBuf = oPart + 32 * PARTS;              // [NG][NODES] node sums / [D][NODES] field of a cell
     static constexpr int nBuf = NG * NODES > D * NODES ? NG * NODES : D * NODES;
     static constexpr int oCol = oBuf + nBuf;                     // [D][ROWS] field on one node column
     static constexpr int warp_elems = (oCol + D * ROWS + 3) / 4 * 4;
@@ -195,7 +199,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
     const int hm = HM ? 1 : g.hmul;
     constexpr int S = SH::S, S2 = S / 2, SZ = SH::SZ, ROWS = SH::ROWS;
     constexpr int G = SH::G, RPL = SH::RPL, NG = SH::NG, NV = SH::NV, NODES = SH::NODES, NPL = SH::NPL;
-    constexpr int WR = SH::WR, RECS = SH::RECS;
+    constexpr int WR = SH::WR, RECS = SH::RECS, PARTS = SH::PARTS;
     constexpr bool DEP = (MODE & kModeDeposit) != 0, PUSH = (MODE & kModePush) != 0;
     constexpr unsigned FULL = 0xFFFFFFFFu;
     constexpr int sh = (S == 4) ? 1 : 0;              // the cell's stencil starts at node column cx - sh
@@ -513,7 +517,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
                 if constexpr (PUSH) {                 // (a repeated record writes the same values again)
 #pragma unroll
                     for (int c = 0; c < D; ++c)
-                        sts1<T>(a_part + (uint32_t)((r * D + c) * G + lg) * B, pk_lo(sum[c]) + pk_hi(sum[c]));
+                        sts1<T>(a_part + (uint32_t)(r * PARTS + c * G + lg) * B, pk_lo(sum[c]) + pk_hi(sum[c]));
                 }
             }
             since += end - pos;
@@ -530,7 +534,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
 #pragma unroll
                 for (int c = 0; c < D; ++c) {
                     T pe[G];
-                    lds<T, G>(a_part + (uint32_t)((idx * D + c) * G) * B, pe);
+                    lds<T, G>(a_part + (uint32_t)(idx * PARTS + c * G) * B, pe);
                     e[c] = pe[0];
 #pragma unroll
                     for (int q = 1; q < G; ++q) e[c] += pe[q];

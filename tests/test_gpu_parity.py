@@ -645,3 +645,35 @@ def test_chain_flag_on_foreign_arrays_falls_back():
     torch.cuda.synchronize()
     assert np.array_equal(st.cell_offsets[: g.cells + 1].cpu().numpy(), ref2["cell_offsets"])
     assert np.array_equal(st.perm[:n].cpu().numpy(), ref2["perm"])
+
+
+@pytest.mark.parametrize("name,kw,mode", [("cfg1", dict(), "plain"), ("cfg3", dict(N=200_000, n=(32, 32, 32)), "plain"),
+                                          ("cfg5", dict(N=8 * 16 ** 3, n=(16, 16, 16)), "closed"),
+                                          ("cfg2", dict(N=100_000, n=(32, 32)), "bucket")])
+def test_graph_replay_equals_plain_stepping(name, kw, mode):
+    """Stepper(graph=True) replays the sort steps from CUDA graphs (launch-bound problems).  Every choice inside a step is
+    made on the device, so the replayed steps must be the plain ones bit for bit -- perm, offsets, x, v, w -- over 7 steps
+    (first sort, pre-ordered sorts, both ping-pong directions)."""
+    _, B = _mods()
+    cfg = _cfg(name, kw)
+    wl = W.make_workload(cfg)
+    g = B.grid_of(cfg)
+    extra = dict(closed_loop=True) if mode == "closed" else (dict(bucket=(4, 2)) if mode == "bucket" else {})
+    a = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, **extra)
+    b = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, graph=True, **extra)
+    for k in range(7):
+        a.step(cfg.dt, cfg.qm, True)
+        b.step(cfg.dt, cfg.qm, True)
+        torch.cuda.synchronize()
+        if mode == "closed":
+            # the field comes from rho, whose reductions have no fixed order: two runs agree to rounding, not bit for bit
+            for c in range(cfg.dim):
+                assert err_x(b.cur["x"][c].cpu().numpy(), a.cur["x"][c].cpu().numpy(), cfg.L[c]) <= 1e-12
+            continue
+        assert torch.equal(a.perm[: cfg.N], b.perm[: cfg.N]), "perm at step %d" % k
+        assert torch.equal(a.cell_offsets, b.cell_offsets)
+        for c in range(cfg.dim):
+            assert torch.equal(a.cur["x"][c], b.cur["x"][c]) and torch.equal(a.cur["v"][c], b.cur["v"][c])
+        assert torch.equal(a.cur["w"], b.cur["w"])
+        assert err_rho(b.rho.cpu().numpy(), a.rho.cpu().numpy()) <= 1e-6
+    assert b.last_launches > 0 and len(b._graphs) == 2
