@@ -56,6 +56,10 @@ namespace pic {
 #ifndef PIC_RUNS_WARPS
 #define PIC_RUNS_WARPS 1        // warps per block (warps are independent)
 #endif
+#ifndef PIC_RUNS_BATCH_UNROLL
+#define PIC_RUNS_BATCH_UNROLL 1   // batches of 32 slots per trip of the outer loop
+#endif
+constexpr int kRunsBatchUnroll = PIC_RUNS_BATCH_UNROLL;
 constexpr int kRunsWarps = PIC_RUNS_WARPS;
 constexpr int kRunsUnroll = PIC_RUNS_UNROLL;
 constexpr int kRunsThreads = 32 * kRunsWarps;
@@ -391,6 +395,7 @@ k_runs(PartP<T> src, PartP<T> dst, const int32_t* __restrict__ perm, GridP<T> g,
     }
     if (32 + lane < cnt) in1 = VIA_PERM ? perm[jl + 32] : (int)jl + 32;
 
+#pragma unroll (kRunsBatchUnroll)
     for (int b0 = 0; b0 < cnt; b0 += 32) {
         const int nb = (cnt - b0 < 32) ? cnt - b0 : 32;
         const bool valid = lane < nb;
