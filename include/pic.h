@@ -198,11 +198,14 @@ int pic_step(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t 
  *   keep their source order inside it (R7; the paper leaves it arbitrary).  bucket_offsets[B+1] is IN/OUT exactly like
  *   pic_sort's cell_offsets (an optional order hint on entry; offsets of the buckets on return).  Workspace:
  *   pic_workspace_bytes() of the grid.
- * pic_step_buckets: sort by bucket, then the same deposit + gather + accel + push pass over the particles in bucket
- *   order; rho, out as in pic_step.  The pass walks runs of equal CELL key; inside a bucket of several cells the order
- *   is the source order, so runs are short and particles alone in their run go the threads-on-particles way
- *   (setrho 3.3.4): the result is exact for every bucket size, the time grows with it (the sweep is in
- *   profiles/ and DESIGN.md).
+ * pic_step_buckets: sort by bucket, then deposit + gather + accel + push in one pass over the particles in bucket
+ *   order; rho, out as in pic_step.  Buckets of at least 27 cells whose grid tile (bucket + stencil halo, rho in double
+ *   and d field components) fits in 160 KB of shared memory take the paper's own CUDA design: a block per bucket stages the
+ *   tile in shared memory, threads on particles add into it atomically and read the field from it, the tile is flushed
+ *   with one global atomic per node (App. B).  Other buckets are walked as runs of equal
+ *   CELL key (short inside a bucket, where the source order is kept), particles alone in their run going the
+ *   threads-on-particles way (setrho 3.3.4).  The result is exact for every bucket size; one cell per
+ *   bucket is by far the fastest on this hardware (the sweep is in profiles/ and DESIGN.md).
  */
 int pic_bucket_count(const pic_grid_t *grid, const int32_t bucket[3] /* host */, int64_t *count /* host, out */);
 int pic_sort_buckets(const pic_grid_t *grid, const int32_t bucket[3] /* host */, const pic_particles_t *in,

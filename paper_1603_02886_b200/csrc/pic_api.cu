@@ -316,7 +316,7 @@ int pic_step_buckets(const pic_grid_t* grid, const int32_t bucket[3], const pic_
     if ((rc = launch_sort(*grid, *in, o, perm, bucket_offsets, sws, false, false, st)) != PIC_OK) return rc;
     bool unit = true;                            // one cell per bucket: this is pic_step(PIC_SORT)
     for (int c = 0; c < grid->dim; ++c) unit = unit && bucket[c] == 1;
-    rc = launch_fused(*grid, *in, o, perm, sws, rho, E, dt, qm, st, unit);
+    rc = launch_fused(*grid, *in, o, perm, sws, rho, E, dt, qm, st, unit, bucket_offsets);
     mark_phase(PIC_PHASE_PUSH, st);
     return rc;
 }

@@ -277,7 +277,7 @@ int launch_push(const pic_grid_t& g, pic_particles_t& p, int order_state, const 
 // cell_sorted = false (with perm): perm groups the particles by bucket only (pic_step_buckets); nothing is emitted.
 int launch_fused(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
                  const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st,
-                 bool cell_sorted = true);
+                 bool cell_sorted = true, const int32_t* key_offsets = nullptr);
 // the collision-free deposit with a fixed order of additions (pic_nodes.cu); p sorted by cell as cell_offsets says
 int launch_deposit_nodes(const pic_grid_t& g, const pic_particles_t& p, const int32_t* cell_offsets, void* rho,
                          const SortWs& ws, cudaStream_t st);

@@ -4,19 +4,35 @@
 // into a frozen given electric field"): rho(x^t) and the push of x^t
 // read the same particle data once.  Kernel: k_runs<MODE = deposit|push> (pic_runs.cuh).
 #include "pic_runs.cuh"
+#include "pic_tile.cuh"
 
 namespace pic {
 
 template <typename T, int D, int P>
 static int fused_impl(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
-                      const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st, bool cell_sorted)
+                      const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st, bool cell_sorted,
+                      const int32_t* key_offsets)
 {
     int64_t C = 1;
     for (int c = 0; c < g.dim; ++c) C *= g.n[c];
     double* racc = sizeof(T) == 8 ? (double*)rho : ws.racc;
     PIC_CUDA_OK(cudaMemsetAsync(racc, 0, sizeof(double) * (size_t)C, st));
     int rc;
-    if (perm && !cell_sorted) {
+    int64_t bucket_cells = 1;
+    for (int c = 0; c < g.dim; ++c) bucket_cells *= ws.bucket ? ws.bucket[c] : 1;
+    // (small buckets: few tile nodes under many particles, the shared-memory atomics of a warp pile up on the same
+    // nodes and the run kernel with strays is faster -- measured crossover near 3^3 cells, profiles/r02_final.md)
+    if (perm && !cell_sorted && key_offsets && ws.bucket && bucket_cells >= 27 && tile_bytes<T>(g, ws.bucket) <= kTileMaxBytes) {
+        // perm groups the particles by BUCKET (pic_step_buckets) and the bucket's grid tile fits in shared memory: the
+        // paper's design, a block per bucket with the tile staged there (pic_tile.cuh).  Same device-side choice between
+        // one pass through perm and reorder-then-in-place as below.
+        PIC_CUDA_OK(cudaMemsetAsync(ws.chain_sig, 0, sizeof(ChainSig), st));
+        rc = launch_bucket_tile<T, D, P, true>(g, ws.bucket, ws.nkeys, src, p, perm, key_offsets, E, racc, dt, qm, st, ws.gate, 0u);
+        if (rc != PIC_OK) return rc;
+        if ((rc = launch_reorder_records(g, src, p, perm, ws.rec_scratch, ws.gate, 1u, st)) != PIC_OK) return rc;
+        rc = launch_bucket_tile<T, D, P, false>(g, ws.bucket, ws.nkeys, p, p, nullptr, key_offsets, E, racc, dt, qm, st, ws.gate, 1u);
+        if (rc != PIC_OK) return rc;
+    } else if (perm && !cell_sorted) {
         // perm groups the particles by BUCKET (pic_step_buckets): inside a bucket of several cells they keep their
         // source order, so a run of equal cell key is short and most particles are alone in theirs.  The same pass;
         // lone particles are set aside for k_strays (threads on particles, setrho 3.3.4), the others
@@ -59,12 +75,13 @@ static int fused_impl(const pic_grid_t& g, const pic_particles_t& src, pic_parti
 
 template <typename T, int D>
 static int fused_order(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
-                       const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st, bool cell_sorted)
+                       const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st, bool cell_sorted,
+                       const int32_t* key_offsets)
 {
     switch (g.order) {
-    case 1: return fused_impl<T, D, 1>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted);
-    case 2: return fused_impl<T, D, 2>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted);
-    default: return fused_impl<T, D, 3>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted);
+    case 1: return fused_impl<T, D, 1>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted, key_offsets);
+    case 2: return fused_impl<T, D, 2>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted, key_offsets);
+    default: return fused_impl<T, D, 3>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted, key_offsets);
     }
 }
 
@@ -115,13 +132,14 @@ int launch_selfconsistent(const pic_grid_t& g, const pic_particles_t& src, pic_p
 }
 
 int launch_fused(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
-                 const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st, bool cell_sorted)
+                 const SortWs& ws, void* rho, const void* const E[3], double dt, double qm, cudaStream_t st, bool cell_sorted,
+                 const int32_t* key_offsets)
 {
     if (g.dtype == PIC_F32)
-        return g.dim == 2 ? fused_order<float, 2>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted)
-                          : fused_order<float, 3>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted);
-    return g.dim == 2 ? fused_order<double, 2>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted)
-                      : fused_order<double, 3>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted);
+        return g.dim == 2 ? fused_order<float, 2>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted, key_offsets)
+                          : fused_order<float, 3>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted, key_offsets);
+    return g.dim == 2 ? fused_order<double, 2>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted, key_offsets)
+                      : fused_order<double, 3>(g, src, p, perm, ws, rho, E, dt, qm, st, cell_sorted, key_offsets);
 }
 
 }  // namespace pic

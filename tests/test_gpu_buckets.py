@@ -125,14 +125,19 @@ STEP_CASES = [
     ("cfg4", 200_007, (32, 32, 32), (2, 2, 2)),
     ("cfg5", 8 * 16 ** 3 + 5, (16, 16, 16), (4, 4, 2)),
     ("cfg1", 100_000, (64, 64), (8, 8)),
-    ("cfg3", 60_000, (16, 16, 16), (16, 16, 16)),   # one bucket: the step runs on the source order
+    ("cfg3", 60_000, (16, 16, 16), (16, 16, 16)),   # one bucket: the step runs on the source order (137 KB tile: still shared memory)
+    ("cfg3", 90_000, (32, 32, 32), (32, 32, 16)),   # tile too large for shared memory: the run kernel with strays takes over
+    ("cfg2", 120_000, (96, 80), (96, 80)),          # the same in 2-D, fp64
+    ("cfg5", 50_000, (12, 10, 14), (5, 3, 4)),      # ragged buckets, quadratic, fp64
+    ("cfg1", 100_000, (64, 64), (64, 32)),          # linear splines, two buckets (R blocks per bucket)
 ]
 
 
 @pytest.mark.parametrize("name,N,n,bucket", STEP_CASES)
 def test_step_buckets_lockstep(name, N, n, bucket):
     """Three steps of pic_step_buckets, each fed the oracle's state: perm / bucket_offsets bit-exact, rho and the
-    advanced particles (in bucket order) within tolerance."""
+    advanced particles (in bucket order) within tolerance.  Buckets whose grid tile fits in shared memory go through the
+    tile kernel (pic_tile.cuh), the others through the run kernel; the first step takes the reorder-first arm of both."""
     O, B = _mods()
     cfg = _cfg(name, N, n=n)
     wl = W.make_workload(cfg)

@@ -79,7 +79,8 @@ def _run_step(B, cfg, wl, garbage, bucket=None, chained_steps=1):
 
 CASES = [("cfg2", 150_003, dict(n=(48, 40)), None), ("cfg3", 120_001, dict(n=(24, 20, 16)), None),
          ("cfg4", 150_000, dict(n=(16, 16, 16)), None), ("cfg5", 8 * 12 ** 3 + 7, dict(n=(12, 12, 12)), None),
-         ("cfg3", 90_001, dict(n=(16, 16, 16)), (4, 2, 2)), ("cfg1", 100_000, dict(), None)]
+         ("cfg3", 90_001, dict(n=(16, 16, 16)), (4, 2, 2)), ("cfg3", 90_001, dict(n=(16, 16, 16)), (4, 4, 2)),     # run kernel / tile kernel
+         ("cfg1", 100_000, dict(), None)]
 
 
 @pytest.mark.parametrize("name,N,kw,bucket", CASES)
