@@ -537,10 +537,13 @@ def run_deposit_compare(B, torch, cfg, g, wl, st, dev, reps=5, nodes=False):
     ws_ = torch.empty_like(a["w"])
     B.pic_sort(g, a["x"], a["v"], a["w"], xs, vs, ws_, st.perm, st.cell_offsets, st.ws)
     t_sorted = timed(lambda: B.pic_deposit(g, xs, ws_, st.rho, B.PIC_ORDER_SORTED, st.cell_offsets, st.ws))
-    t_nodes = None
+    t_nodes = t_repl = None
     if nodes:      # the collision-free, bitwise reproducible alternative (threads on splines)
         reps, keep = 2, reps
         t_nodes = timed(lambda: B.pic_deposit_nodes(g, xs, ws_, st.rho, st.cell_offsets, st.ws))
+        wsr = torch.empty(B.pic_deposit_replicated_bytes(g, cfg.N), dtype=torch.uint8, device=dev)
+        t_repl = timed(lambda: B.pic_deposit_replicated(g, xs, ws_, st.rho, st.cell_offsets, wsr))
+        del wsr
         reps = keep
     del vs
     x0 = [torch.from_numpy(np.ascontiguousarray(t)).to(dev) for t in wl.x]
@@ -549,6 +552,7 @@ def run_deposit_compare(B, torch, cfg, g, wl, st, dev, reps=5, nodes=False):
     out = {"sorted": t_sorted, "never_sorted": t_unsorted, "unit": "ms per deposit of all particles"}
     if t_nodes is not None:
         out["nodes_deterministic"] = t_nodes
+        out["replicated_deterministic"] = t_repl
     return out
 
 

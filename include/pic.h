@@ -140,6 +140,21 @@ int pic_deposit_nodes(const pic_grid_t *grid, const pic_particles_t *p, const in
                       void *rho, void *ws, size_t ws_bytes, void *stream);
 
 /*
+ * pic_deposit_replicated -- the same rho by the paper's other collision-free algorithm, "threads on buckets with data
+ * replication" (section 3.3.3, Fig. 7): the threads are associated with the buckets
+ * (here: cells) of sorted particles, each sums its particles onto a LOCAL grid of its own -- the cell's nodes plus the guard
+ * nodes its stencils reach -- kept in a temporary global array "without atomics in global memory"; in a second step
+ * "threads are assigned to the grid and collect the data from the temporary variables".  No atomic operation anywhere
+ * and a fixed order of additions (per cell in particle order, then the cells around a node in ascending order): bitwise
+ * reproducible; equal to pic_deposit within rounding.  p sorted by cell, cell_offsets from pic_sort; if they do not
+ * describe the order (checked on the device) the any-order kernel answers instead.
+ * ws: pic_deposit_replicated_bytes() = pic_workspace_bytes() + (4 or 2)^dim doubles per cell.  rho[C] is overwritten.
+ */
+int pic_deposit_replicated_bytes(const pic_grid_t *grid, int64_t n, size_t *bytes /* host, out */);
+int pic_deposit_replicated(const pic_grid_t *grid, const pic_particles_t *p, const int32_t *cell_offsets,
+                           void *rho, void *ws, size_t ws_bytes, void *stream);
+
+/*
  * pic_push -- field gather + accel + push in one pass (rows a6-a7; PAPER.md:82-83 steps iii-iv,
  * 86, 88; models PAPER.md:312, 316):
  *   E_i = sum_j E[j] * prod_c W_p(x_ic/h_c - j_c)   (same splines as the deposit)

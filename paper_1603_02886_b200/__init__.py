@@ -22,7 +22,7 @@ PIC_SORT, PIC_SORT_CHAINED = 1, 3
 
 EXPORTS = ("pic_workspace_bytes", "pic_sort", "pic_deposit", "pic_push", "pic_step",
            "pic_step_host_bytes", "pic_step_host", "pic_step_fields_host_bytes", "pic_step_fields_host",
-           "pic_bucket_count", "pic_sort_buckets", "pic_step_buckets", "pic_deposit_nodes",
+           "pic_bucket_count", "pic_sort_buckets", "pic_step_buckets", "pic_deposit_nodes", "pic_deposit_replicated_bytes", "pic_deposit_replicated",
            "pic_field_solve_bytes", "pic_field_solve", "pic_step_selfconsistent_bytes", "pic_step_selfconsistent",
            "pic_last_launch_count", "pic_set_phase_events",
            "pic_strerror")
@@ -82,6 +82,8 @@ def lib():
         L.pic_sort_buckets.argtypes = [G, B3, P, P, vp, vp, vp, sz, vp]
         L.pic_step_buckets.argtypes = [G, B3, P, P, vp, vp, vp, E3, dbl, dbl, vp, sz, vp]
         L.pic_deposit_nodes.argtypes = [G, P, vp, vp, vp, sz, vp]
+        L.pic_deposit_replicated_bytes.argtypes = [G, i64, ctypes.POINTER(sz)]
+        L.pic_deposit_replicated.argtypes = [G, P, vp, vp, vp, sz, vp]
         L.pic_field_solve_bytes.argtypes = [G, ctypes.POINTER(sz)]
         L.pic_field_solve.argtypes = [G, vp, E3, vp, vp, sz, vp]
         L.pic_step_selfconsistent_bytes.argtypes = [G, i64, ctypes.POINTER(sz)]
@@ -284,6 +286,24 @@ def pic_deposit_nodes(g: Grid, x, w, rho, cell_offsets, ws, stream=None):
     p = _particles(g, x, None, w, n)
     _check(lib().pic_deposit_nodes(ctypes.byref(cg), ctypes.byref(p), _ptr(cell_offsets), _ptr(rho), _ptr(ws),
                                    ws.numel() * ws.element_size(), _stream(stream)), "pic_deposit_nodes")
+
+
+def pic_deposit_replicated_bytes(g: Grid, n: int) -> int:
+    cg, out = g.c(), ctypes.c_size_t(0)
+    _check(lib().pic_deposit_replicated_bytes(ctypes.byref(cg), n, ctypes.byref(out)), "pic_deposit_replicated_bytes")
+    return int(out.value)
+
+
+def pic_deposit_replicated(g: Grid, x, w, rho, cell_offsets, ws, stream=None):
+    """rho[C] by per-cell local grids and a per-node assembly (setrho 3.3.3): no atomics, bitwise reproducible.
+    x, w sorted by cell; cell_offsets from pic_sort; ws of pic_deposit_replicated_bytes()."""
+    n = w.numel()
+    _dev_check(g, list(x) + [w], n)
+    _dev_check(g, [rho], g.cells)
+    cg = g.c()
+    p = _particles(g, x, None, w, n)
+    _check(lib().pic_deposit_replicated(ctypes.byref(cg), ctypes.byref(p), _ptr(cell_offsets), _ptr(rho), _ptr(ws),
+                                        ws.numel() * ws.element_size(), _stream(stream)), "pic_deposit_replicated")
 
 
 def pic_field_solve_bytes(g: Grid) -> int:

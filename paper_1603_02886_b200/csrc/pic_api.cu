@@ -193,6 +193,33 @@ int pic_deposit_nodes(const pic_grid_t* grid, const pic_particles_t* p, const in
     return rc;
 }
 
+int pic_deposit_replicated_bytes(const pic_grid_t* grid, int64_t n, size_t* bytes)
+{
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if (!bytes || n < 0 || n >= ((int64_t)1 << 30)) return PIC_ERR_INVALID_ARG;
+    *bytes = sort_ws_bytes(*grid, n) + replicated_slab_bytes(*grid);
+    return PIC_OK;
+}
+
+int pic_deposit_replicated(const pic_grid_t* grid, const pic_particles_t* p, const int32_t* cell_offsets, void* rho, void* ws,
+                           size_t ws_bytes, void* stream)
+{
+    g_launches = 0;
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if ((rc = check_particles(*grid, p, false, true)) != PIC_OK) return rc;
+    if (!aligned16(cell_offsets) || !aligned16(rho) || !aligned16(ws)) return PIC_ERR_INVALID_ARG;
+    const size_t sb = sort_ws_bytes(*grid, p->n);
+    if (ws_bytes < sb + replicated_slab_bytes(*grid)) return PIC_ERR_WORKSPACE;
+    SortWs sws;
+    if ((rc = carve_sort_ws(*grid, p->n, ws, sb, sws)) != PIC_OK) return rc;
+    mark_phase(PIC_PHASE_BEGIN, (cudaStream_t)stream);
+    rc = launch_deposit_replicated(*grid, *p, cell_offsets, rho, sws, (char*)ws + sb, (cudaStream_t)stream);
+    mark_phase(PIC_PHASE_DEPOSIT, (cudaStream_t)stream);
+    return rc;
+}
+
 int pic_push(const pic_grid_t* grid, pic_particles_t* p, int order_state, const int32_t* cell_offsets,
              const void* const E[3], double dt, double qm, void* stream)
 {

@@ -287,6 +287,10 @@ int launch_field_solve(const pic_grid_t& g, const void* rho, void* const E[3], v
 // the closed loop i-iv: deposit along perm (+ reorder into p), field solve, gather + accel + push in place
 int launch_selfconsistent(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,
                           const SortWs& ws, void* rho, void* const E[3], void* field_ws, double dt, double qm, cudaStream_t st);
+// deposit by replication (setrho 3.3.3): per-cell local grids in `slab` (replicated_slab_bytes), then assembly per node
+size_t replicated_slab_bytes(const pic_grid_t& g);
+int launch_deposit_replicated(const pic_grid_t& g, const pic_particles_t& p, const int32_t* cell_offsets, void* rho,
+                              const SortWs& ws, void* slab, cudaStream_t st);
 // out_a[j] = in_a[perm[j]] for every attribute; runs only if *gate == want (gate may be NULL)
 int launch_reorder(const pic_grid_t& g, const pic_particles_t& in, const pic_particles_t& out, const int32_t* perm,
                    const uint32_t* gate, uint32_t want, cudaStream_t st);

@@ -275,4 +275,160 @@ int launch_deposit_nodes(const pic_grid_t& g, const pic_particles_t& p, const in
     return g.dim == 2 ? nodes_order<double, 2>(g, p, cell_offsets, rho, ws, st) : nodes_order<double, 3>(g, p, cell_offsets, rho, ws, st);
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// pic_deposit_replicated: "collision-free: threads on buckets with data replication" (section 3.3.3,
+// Fig. 7): "replicate the grid data from global to local data and sort particles in buckets ... associating threads
+// with buckets of particles.  This ensures that each thread does the charge assignment on its local grid thus preventing
+// race condition.  Guard-cells ... provide temporary memory for data exchange ... In the first step, reduction can be
+// applied to local temporary variables without atomics in global memory.  In the second step, threads are assigned to
+// the grid and collect the data from the temporary variables in global memory."  One cell per bucket:
+//   k_deposit_cells_private  one thread per cell: its particles in order, the S^d nodes of the cell's stencil (the local
+//                            grid with its guard nodes) summed in registers in double, written to slab[cell][S^d]
+//   k_assemble_nodes         one thread per node: the local-grid entries of the cells around it, in ascending cell order
+// No atomic anywhere, fixed order everywhere: bitwise reproducible.  (The association differs from the particle-order sum
+// of pic_deposit_nodes: sums per cell first.)  Wrong offsets are found on the device and answered by the any-order kernel.
+template <typename T, int D, int P>
+__global__ void __launch_bounds__(64) k_deposit_cells_private(PartP<T> p, GridP<T> g, const int32_t* __restrict__ off, int64_t C,
+                                                              double inv_vol, double* __restrict__ slab, uint32_t* __restrict__ bad)
+{
+    if (*bad) return;
+    constexpr int S = StencilW<P>::S, SZ = (D == 3) ? S : 1;
+    const int64_t cell = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= C) return;
+    int cc[3];
+    cc[0] = (int)(cell % g.n[0]);
+    cc[1] = (int)((cell / g.n[0]) % g.n[1]);
+    cc[2] = (D == 3) ? (int)(cell / ((int64_t)g.n[0] * g.n[1])) : 0;
+    double acc[SZ][S][S];
+#pragma unroll
+    for (int a = 0; a < SZ; ++a)
+#pragma unroll
+        for (int b = 0; b < S; ++b)
+#pragma unroll
+            for (int c = 0; c < S; ++c) acc[a][b][c] = 0.0;
+    bool wrong = false;
+    const int32_t end = off[cell + 1];
+    for (int32_t i = off[cell]; i < end; ++i) {
+        double w[3][S];
+#pragma unroll
+        for (int c = 0; c < D; ++c) {
+            T wt[S];
+            const int i0 = cell_weights<T, P>(p.x[c][i], g.h[c], g.inv_h[c], g.hmul, g.n[c], wt);
+            if (i0 != cc[c]) wrong = true;
+#pragma unroll
+            for (int a = 0; a < S; ++a) w[c][a] = (double)wt[a];
+        }
+        const double q = (double)p.w[i] * inv_vol;
+#pragma unroll
+        for (int a = 0; a < SZ; ++a) {
+            const double qz = (D == 3) ? q * w[2][a] : q;
+#pragma unroll
+            for (int b = 0; b < S; ++b) {
+                const double qy = qz * w[1][b];
+#pragma unroll
+                for (int c = 0; c < S; ++c) acc[a][b][c] = fma(qy, w[0][c], acc[a][b][c]);
+            }
+        }
+    }
+    double* mine = slab + cell * (int64_t)(SZ * S * S);
+#pragma unroll
+    for (int a = 0; a < SZ; ++a)
+#pragma unroll
+        for (int b = 0; b < S; ++b)
+#pragma unroll
+            for (int c = 0; c < S; ++c) mine[(a * S + b) * S + c] = acc[a][b][c];
+    if (wrong) *bad = 1u;
+}
+
+// (cell, local index) pairs of one dimension whose local grid holds node j, ascending by cell then by index; at most 2 S
+template <int P>
+__device__ __forceinline__ int node_sources(int j, int n, int (&cell)[8], int (&loc)[8])
+{
+    constexpr int S = StencilW<P>::S, sh = (S == 4) ? 1 : 0;
+    const NodeCells<P> nc(j, n);
+    int m = 0;
+    for (int q = 0; q < nc.m; ++q) {
+        const int c = nc.cell(q);
+        for (int a = 0; a < S; ++a)
+            if (fold(c - sh + a, n) == j && m < 8) { cell[m] = c; loc[m] = a; ++m; }
+    }
+    return m;
+}
+
+template <typename T, int D, int P>
+__global__ void __launch_bounds__(128) k_assemble_nodes(GridP<T> g, int64_t C, const double* __restrict__ slab, T* __restrict__ rho,
+                                                        const uint32_t* __restrict__ bad)
+{
+    if (*bad) return;
+    constexpr int S = StencilW<P>::S, SZ = (D == 3) ? S : 1;
+    const int64_t node = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= C) return;
+    const int jx = (int)(node % g.n[0]), jy = (int)((node / g.n[0]) % g.n[1]);
+    const int jz = (D == 3) ? (int)(node / ((int64_t)g.n[0] * g.n[1])) : 0;
+    int cx[8], ax[8], cy[8], ay[8], cz[8] = {0, 0, 0, 0, 0, 0, 0, 0}, az[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const int mx = node_sources<P>(jx, g.n[0], cx, ax), my = node_sources<P>(jy, g.n[1], cy, ay);
+    const int mz = (D == 3) ? node_sources<P>(jz, g.n[2], cz, az) : 1;
+    double acc = 0.0;
+    for (int a = 0; a < mz; ++a)
+        for (int b = 0; b < my; ++b)
+            for (int c = 0; c < mx; ++c) {
+                const int64_t cell = cx[c] + (int64_t)g.n[0] * (cy[b] + (int64_t)g.n[1] * cz[a]);
+                acc += slab[cell * (int64_t)(SZ * S * S) + (az[a] * S + ay[b]) * S + ax[c]];
+            }
+    rho[node] = (T)acc;
+}
+
+size_t replicated_slab_bytes(const pic_grid_t& g)
+{
+    size_t C = 1, per = 1;
+    const int S = g.order == 1 ? 2 : 4;
+    for (int c = 0; c < g.dim; ++c) { C *= (size_t)g.n[c]; per *= (size_t)S; }
+    return (C * per * sizeof(double) + 255) & ~(size_t)255;
+}
+
+template <typename T, int D, int P>
+static int replicated_impl(const pic_grid_t& g, const pic_particles_t& p, const int32_t* off, void* rho, const SortWs& ws,
+                           double* slab, cudaStream_t st)
+{
+    int64_t C = 1;
+    double inv_vol = 1.0;
+    for (int c = 0; c < g.dim; ++c) { C *= g.n[c]; inv_vol /= g.h[c]; }
+    uint32_t* bad = ws.counters + kCtrNodesBad;
+    PIC_CUDA_OK(cudaMemsetAsync(bad, 0, 2 * sizeof(uint32_t), st));
+    k_offsets_check<<<(unsigned)((C + 1 + 255) / 256), 256, 0, st>>>(off, (int)C, p.n, bad);
+    const GridP<T> gp = make_gridp<T>(g);
+    k_deposit_cells_private<T, D, P><<<(unsigned)((C + 63) / 64), 64, 0, st>>>(make_partp<T>(p), gp, off, C, inv_vol, slab, bad);
+    k_assemble_nodes<T, D, P><<<(unsigned)((C + 127) / 128), 128, 0, st>>>(gp, C, slab, (T*)rho, bad);
+    count_launch(3);
+    PIC_CUDA_OK(cudaMemsetAsync(ws.racc, 0, sizeof(double) * (size_t)C, st));
+    if (p.n > 0) {
+        int rc = launch_runs<T, D, P, kModeDeposit, false>(g, p, p, nullptr, nullptr, ws.racc, 0.0, 0.0, st, bad, 1u);
+        if (rc != PIC_OK) return rc;
+    }
+    k_round_rho_gated<T><<<(unsigned)((C + 255) / 256), 256, 0, st>>>(ws.racc, (T*)rho, C, bad, 1u);
+    count_launch();
+    return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+}
+
+template <typename T, int D>
+static int replicated_order(const pic_grid_t& g, const pic_particles_t& p, const int32_t* off, void* rho, const SortWs& ws,
+                            double* slab, cudaStream_t st)
+{
+    switch (g.order) {
+    case 1: return replicated_impl<T, D, 1>(g, p, off, rho, ws, slab, st);
+    case 2: return replicated_impl<T, D, 2>(g, p, off, rho, ws, slab, st);
+    default: return replicated_impl<T, D, 3>(g, p, off, rho, ws, slab, st);
+    }
+}
+
+int launch_deposit_replicated(const pic_grid_t& g, const pic_particles_t& p, const int32_t* cell_offsets, void* rho,
+                              const SortWs& ws, void* slab, cudaStream_t st)
+{
+    if (g.dtype == PIC_F32)
+        return g.dim == 2 ? replicated_order<float, 2>(g, p, cell_offsets, rho, ws, (double*)slab, st)
+                          : replicated_order<float, 3>(g, p, cell_offsets, rho, ws, (double*)slab, st);
+    return g.dim == 2 ? replicated_order<double, 2>(g, p, cell_offsets, rho, ws, (double*)slab, st)
+                      : replicated_order<double, 3>(g, p, cell_offsets, rho, ws, (double*)slab, st);
+}
+
 }  // namespace pic

@@ -139,3 +139,63 @@ def test_nodes_offsets_that_do_not_describe_the_order(what):
     ref = O.deposit(go, x, w)
     got = _gpu_nodes(B, B.grid_of(cfg), x, w, np.asarray(o))
     assert err_rho(got, ref) <= TOL_RHO[cfg.dtype]
+
+
+# ---- pic_deposit_replicated: threads on buckets with data replication (setrho 3.3.3) ----------------
+def _gpu_replicated(B, g, xs, wsrt, off):
+    n = wsrt.shape[0]
+    x = to_dev(xs)
+    w = to_dev([wsrt])[0]
+    offd = torch.from_numpy(np.concatenate([off.astype(np.int32), np.zeros(3, np.int32)])).cuda()
+    rho = torch.full((g.cells,), float("nan"), dtype=g.torch_dtype, device="cuda")
+    ws = torch.full((B.pic_deposit_replicated_bytes(g, n),), 0xA5, dtype=torch.uint8, device="cuda")
+    B.pic_deposit_replicated(g, x, w, rho, offd, ws)
+    torch.cuda.synchronize()
+    return rho.cpu().numpy()
+
+
+@pytest.mark.parametrize("name,N,kw,order,dtype", CASES)
+def test_replicated_parity_and_reproducibility(name, N, kw, order, dtype):
+    """Within the deposit tolerance of the oracle (the association differs: sums per cell first), and bit-identical from run
+    to run (no atomics, fixed order)."""
+    O, B = _mods()
+    cfg = W.CONFIGS[name].scaled(N, order=order, dtype=dtype, **kw)
+    xs, wsrt, off = _sorted_inputs(O, cfg)
+    ref = O.deposit(O.grid_of(cfg), xs, wsrt)
+    got = _gpu_replicated(B, B.grid_of(cfg), xs, wsrt, off)
+    assert err_rho(got, ref) <= TOL_RHO[dtype]
+    again = _gpu_replicated(B, B.grid_of(cfg), xs, wsrt, off)
+    assert np.array_equal(_bits(got), _bits(again))
+    scale = np.prod([cfg.h] * cfg.dim)
+    assert abs(np.sum(got.astype(np.float64)) * scale - np.sum(wsrt.astype(np.float64))) <= (1e-12 if dtype == "f64" else 2e-6) * np.sum(np.abs(wsrt))
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_replicated_clustered_and_spacing(dtype):
+    O, B = _mods()
+    for cfg in (W.CONFIGS["cfg4"].scaled(400_000, n=(16, 16, 16), dtype=dtype),
+                W.CONFIGS["cfg3"].scaled(50_000, n=(12, 10, 14), h=0.3, order=2, dtype=dtype)):
+        xs, wsrt, off = _sorted_inputs(O, cfg)
+        ref = O.deposit(O.grid_of(cfg), xs, wsrt)
+        got = _gpu_replicated(B, B.grid_of(cfg), xs, wsrt, off)
+        assert err_rho(got, ref) <= TOL_RHO[dtype]
+
+
+@pytest.mark.parametrize("what", ["unsorted", "garbage", "shifted"])
+def test_replicated_offsets_that_do_not_describe_the_order(what):
+    O, B = _mods()
+    cfg = W.CONFIGS["cfg3"].scaled(80_000, n=(16, 16, 16))
+    wl = W.make_workload(cfg)
+    go = O.grid_of(cfg)
+    xs, vs, wsrt, perm, off = O.sort(go, wl.x, wl.v, wl.w)
+    if what == "unsorted":
+        x, w, o = wl.x, wl.w, off
+    elif what == "garbage":
+        x, w, o = xs, wsrt, np.random.default_rng(3).integers(-10, cfg.N + 10, off.size)
+    else:
+        x, w = xs, wsrt
+        o = np.minimum(off + 1, cfg.N)
+        o[0] = 0
+    ref = O.deposit(go, x, w)
+    got = _gpu_replicated(B, B.grid_of(cfg), x, w, np.asarray(o))
+    assert err_rho(got, ref) <= TOL_RHO[cfg.dtype]
