@@ -82,3 +82,24 @@ def test_product_does_not_import_the_oracle():
         if f.endswith((".py", ".c", ".h")):
             s = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_1603_02886_b200" not in s and "csrc" not in s, f
+
+
+def test_host_only_entry_points_of_the_next_rows(B):
+    """Pure host computations of the NEXT rows: bucket counts, workspace sizes, argument validation (no kernel runs)."""
+    g = B.Grid(3, (128, 128, 128), (1.0, 1.0, 1.0), 3, "f32")
+    assert B.pic_bucket_count(g, (1, 1, 1)) == 128 ** 3
+    assert B.pic_bucket_count(g, (4, 4, 4)) == 32 ** 3
+    assert B.pic_bucket_count(g, (5, 128, 3)) == 26 * 1 * 43          # ragged last buckets
+    for bad in ((0, 1, 1), (1, 129, 1), (1, 1, -2)):
+        with pytest.raises(B.PicError, match="invalid argument"):
+            B.pic_bucket_count(g, bad)
+    C = 128 ** 3
+    assert B.pic_field_solve_bytes(g) >= 2 * 16 * C                   # two complex-double grids
+    n = 1_000_000
+    base = B.pic_workspace_bytes(g, n)
+    assert B.pic_step_selfconsistent_bytes(g, n) == base + B.pic_field_solve_bytes(g)
+    assert B.pic_deposit_replicated_bytes(g, n) == base + 64 * 8 * C  # 4^3 local-grid nodes per cell, double
+    g2 = B.Grid(2, (64, 32), (1.0, 1.0), 1, "f64")
+    assert B.pic_deposit_replicated_bytes(g2, 10) == B.pic_workspace_bytes(g2, 10) + 4 * 8 * 64 * 32
+    with pytest.raises(B.PicError):
+        B.pic_deposit_replicated_bytes(g, 2 ** 30)
