@@ -21,14 +21,19 @@
 //   * the full-key histogram and its exclusive scan give cell_offsets; the movers' histogram and
 //     its scan place each mover inside its cell.
 //
-// Kernels:  k_hint_check     hint -> private copy, validity flag
-//           k_classify       x[d] -> key, histograms, stayer/mover split, movers compacted in order
+// Kernels:  k_hint_check     hint -> private copy, validity flag; is this call the next link of a chain?
+//           k_classify       x[d] -> key (cell or bucket), histograms, stayer/mover split, movers staged per 2048 positions
+//                            (returns at once in a chain: the previous step kernel has emitted all of it)
+//           k_chain_counts   in a chain: the three histograms from the step kernel's per-cell in/out counters
 //           k_scan_cells     count[C] -> exclusive offsets [C+1] (single pass, decoupled look-back)
+//           k_movers_place   staged movers -> one list in position order
 //           k_scan_digits    digit histograms -> exclusive global digit offsets
-//           k_radix_pass     one stable partition of the movers by an (at most) 8-bit digit
+//           k_radix_pass     one stable partition of the movers by an (at most) 8-bit digit; the last pass writes
+//                            the movers' entries of perm
 //           k_cell_base      per cell: where its stayers start in perm
-//           k_perm_stayers   perm of the stayers (the movers' entries come from the last radix pass)
-//           k_reorder        out_a[j] = in_a[perm[j]] for every attribute (pic_sort only)
+//           k_perm_stayers   perm of the stayers
+//           k_reorder        out_a[j] = in_a[perm[j]] value by value (most particles stay where they are)
+//           k_pack16/unpack16  the same through 16-byte records (most particles move: first sort)
 #include <cmath>
 #include <cstring>
 

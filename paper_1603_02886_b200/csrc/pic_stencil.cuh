@@ -1,5 +1,5 @@
 // pic_stencil.cuh -- pieces shared by the kernels that work on particles grouped by cell
-// (pic_rows.cuh) and by the any-order kernels: field pointers, kernel modes, the
+// (pic_runs.cuh, pic_tile.cuh, pic_nodes.cu) and by the any-order kernels: field pointers, kernel modes, the
 // stencil width of a cell, packed pairs, the 1-D spline weights of a cell's stencil.
 //
 // S = stencil width of a CELL: 2 for p = 1, 4 for p = 2, 3 (a quadratic particle touches 3 of the
