@@ -238,7 +238,7 @@ struct SortWs {
     uint32_t* gate;          // one word of counters: 1 = more than half of the particles are movers (set by the sort)
     uint32_t* stray_count;   // one word of counters: particles the step kernel has set aside (zeroed with the counters)
     uint32_t* stray_list;    // [N] their slots (= idx[0]: free once perm is written)
-    void* rec_scratch;       // 16 N bytes (keys and idx arrays: free once perm is written) for launch_reorder_records
+    void* rec_scratch;       // 32 N bytes (keys, idx, pkey arrays: free once perm is written; + 12 N) for launch_reorder_records
     double* racc;            // [C] double accumulation grid of the deposit (not in the zero region)
     int32_t* prev_off;       // [C+1] cell_offsets as the last sort of a chain wrote them (the next one's hint)
     ChainSig* chain_sig;     // what that step worked on
@@ -294,7 +294,7 @@ int launch_deposit_replicated(const pic_grid_t& g, const pic_particles_t& p, con
 // out_a[j] = in_a[perm[j]] for every attribute; runs only if *gate == want (gate may be NULL)
 int launch_reorder(const pic_grid_t& g, const pic_particles_t& in, const pic_particles_t& out, const int32_t* perm,
                    const uint32_t* gate, uint32_t want, cudaStream_t st);
-// the same through 16-byte records of interleaved attributes (for a nearly random perm); scratch: 16 N bytes
+// the same through 32-byte records of interleaved attributes (for a nearly random perm); scratch: 32 N bytes
 int launch_reorder_records(const pic_grid_t& g, const pic_particles_t& in, const pic_particles_t& out, const int32_t* perm,
                            void* scratch, const uint32_t* gate, uint32_t want, cudaStream_t st);
 

@@ -33,7 +33,7 @@
 //           k_cell_base      per cell: where its stayers start in perm
 //           k_perm_stayers   perm of the stayers
 //           k_reorder        out_a[j] = in_a[perm[j]] value by value (most particles stay where they are)
-//           k_pack16/unpack16  the same through 16-byte records (most particles move: first sort)
+//           k_pack_rec/k_unpack_rec  the same through 32-byte records (most particles move: first sort)
 #include <cmath>
 #include <cstring>
 
@@ -718,45 +718,50 @@ __global__ void __launch_bounds__(256) k_reorder(PartP<T> in, PartP<T> out, cons
 
 // The same reorder when perm is (nearly) random -- the first sort of particles in random order.  k_reorder then
 // fetches one 32-byte sector per 4- or 8-byte value: A sectors per particle (16.4 ms for 1e8 fp32 particles, 3-D).
-// Here 16 bytes of attributes travel together: K = 16/sizeof(T) attribute arrays are interleaved into 16-byte
-// records (coalesced both ways), then slot j fetches record perm[j] with ONE scattered access and writes its K
-// attributes (coalesced).  ceil(A/K) rounds through a 16 N byte scratch (the movers' key/index arrays, free once
-// perm exists).  "Scattered ... a multiple of 32 bytes for every moved particle" is the paper's cost of moving a
-// particle: this keeps it at one such access per 16 bytes instead of one per value.
+// Here a whole sector of attributes travels together: K = 32/sizeof(T) attribute arrays are interleaved into 32-byte
+// records (coalesced both ways), then slot j fetches record perm[j] with ONE scattered sector and writes its K
+// attributes (coalesced).  ceil(A/K) rounds (one in fp32, two in fp64) through a 32 N byte scratch (the movers'
+// key/index arrays and the per-position keys, free once perm exists, plus 12 N bytes of their own).  "Scattered ... a
+// multiple of 32 bytes for every moved particle" is the paper's cost of moving a particle: this keeps
+// it at one such access per particle (fp32) instead of one per value.
 template <typename T>
-__global__ void __launch_bounds__(256) k_pack16(const T* __restrict__ a0, const T* __restrict__ a1, const T* __restrict__ a2,
-                                                const T* __restrict__ a3, uint4* __restrict__ rec, int64_t n,
-                                                const uint32_t* __restrict__ gate, uint32_t want)
+struct RecPtrs {
+    const T* s[8];
+    T* d[8];
+};
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_pack_rec(RecPtrs<T> a, uint4* __restrict__ rec, int64_t n,
+                                                  const uint32_t* __restrict__ gate, uint32_t want)
 {
     if (gate && *gate != want) return;
+    constexpr int K = 32 / (int)sizeof(T);
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        union { uint4 q; T v[16 / sizeof(T)]; } r;
-        r.q = make_uint4(0u, 0u, 0u, 0u);
-        r.v[0] = a0[i];
-        if (a1) r.v[1] = a1[i];
-        if constexpr (sizeof(T) == 4) {
-            if (a2) r.v[2] = a2[i];
-            if (a3) r.v[3] = a3[i];
-        }
-        rec[i] = r.q;
+        union { uint4 q[2]; T v[K]; } r;
+        r.q[0] = make_uint4(0u, 0u, 0u, 0u);
+        r.q[1] = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+            if (a.s[k]) r.v[k] = a.s[k][i];
+        rec[2 * i] = r.q[0];
+        rec[2 * i + 1] = r.q[1];
     }
 }
 
 template <typename T>
-__global__ void __launch_bounds__(256) k_unpack16(const uint4* __restrict__ rec, const int32_t* __restrict__ perm, T* __restrict__ o0,
-                                                  T* __restrict__ o1, T* __restrict__ o2, T* __restrict__ o3, int64_t n,
-                                                  const uint32_t* __restrict__ gate, uint32_t want)
+__global__ void __launch_bounds__(256) k_unpack_rec(RecPtrs<T> a, const uint4* __restrict__ rec, const int32_t* __restrict__ perm,
+                                                    int64_t n, const uint32_t* __restrict__ gate, uint32_t want)
 {
     if (gate && *gate != want) return;
+    constexpr int K = 32 / (int)sizeof(T);
     for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += (int64_t)gridDim.x * blockDim.x) {
-        union { uint4 q; T v[16 / sizeof(T)]; } r;
-        r.q = __ldg(rec + perm[j]);
-        o0[j] = r.v[0];
-        if (o1) o1[j] = r.v[1];
-        if constexpr (sizeof(T) == 4) {
-            if (o2) o2[j] = r.v[2];
-            if (o3) o3[j] = r.v[3];
-        }
+        const int64_t i = perm[j];
+        union { uint4 q[2]; T v[K]; } r;
+        r.q[0] = __ldg(rec + 2 * i);
+        r.q[1] = __ldg(rec + 2 * i + 1);
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+            if (a.d[k]) a.d[k][j] = r.v[k];
     }
 }
 
@@ -765,7 +770,7 @@ static int reorder_records(const pic_grid_t& g, const pic_particles_t& in, const
                            void* scratch, const uint32_t* gate, uint32_t want, cudaStream_t st)
 {
     const int64_t n = in.n;
-    constexpr int K = 16 / sizeof(T);
+    constexpr int K = 32 / (int)sizeof(T);
     const T* src[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     T* dst[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     int A = 0;
@@ -775,17 +780,20 @@ static int reorder_records(const pic_grid_t& g, const pic_particles_t& in, const
     const int64_t want_blocks = (n + 255) / 256, cap = (int64_t)sm_count() * 8;
     const unsigned blocks = (unsigned)(want_blocks < cap ? want_blocks : cap);
     for (int a = 0; a < A; a += K) {
-        const T* s4[4] = {nullptr, nullptr, nullptr, nullptr};
-        T* d4[4] = {nullptr, nullptr, nullptr, nullptr};
-        for (int k = 0; k < K && a + k < A; ++k) { s4[k] = src[a + k]; d4[k] = dst[a + k]; }
-        k_pack16<T><<<blocks, 256, 0, st>>>(s4[0], s4[1], s4[2], s4[3], (uint4*)scratch, n, gate, want);
-        k_unpack16<T><<<blocks, 256, 0, st>>>((const uint4*)scratch, perm, d4[0], d4[1], d4[2], d4[3], n, gate, want);
+        RecPtrs<T> rp;
+        for (int k = 0; k < 8; ++k) {
+            const bool on = k < K && a + k < A;
+            rp.s[k] = on ? src[a + k] : nullptr;
+            rp.d[k] = on ? dst[a + k] : nullptr;
+        }
+        k_pack_rec<T><<<blocks, 256, 0, st>>>(rp, (uint4*)scratch, n, gate, want);
+        k_unpack_rec<T><<<blocks, 256, 0, st>>>(rp, (const uint4*)scratch, perm, n, gate, want);
         count_launch(2);
     }
     return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
 }
 
-// out_a[j] = in_a[perm[j]] when *gate == want, through 16-byte records (see k_pack16); scratch: 16 N bytes
+// out_a[j] = in_a[perm[j]] when *gate == want, through 32-byte records (see k_pack_rec); scratch: 32 N bytes
 int launch_reorder_records(const pic_grid_t& g, const pic_particles_t& in, const pic_particles_t& out, const int32_t* perm,
                            void* scratch, const uint32_t* gate, uint32_t want, cudaStream_t st)
 {
@@ -812,7 +820,7 @@ static int64_t cells_of(const pic_grid_t& g)
 }
 
 struct SortLayout {
-    size_t keys0, keys1, idx0, idx1, pkey, mask, mprefix, old_off, prev_off, mover_off, cell_base, tile_count, tile_base, lookback;
+    size_t keys0, keys1, idx0, idx1, pkey, rec_extra, mask, mprefix, old_off, prev_off, mover_off, cell_base, tile_count, tile_base, lookback;
     size_t hist_begin, cell_count, mover_count, mover_lo, hist_end, emit_begin, cell_out, mover_in, emit_end;
     size_t zero_begin, digit_hist, scan_status, cls_status, counters, zero_end;
     size_t chain_sig, racc, total;
@@ -840,6 +848,7 @@ static SortLayout sort_layout(const pic_grid_t& g, int64_t n)
     L.idx0 = off; off += nb;
     L.idx1 = off; off += nb;
     L.pkey = off; off += nb;
+    L.rec_extra = off; off += align256(12 * (size_t)(n > 0 ? n : 1));      // keys0 .. here: the 32 N byte record scratch
     L.mask = off; off += wb;
     L.mprefix = off; off += wb;
     L.old_off = off; off += cb;
@@ -925,7 +934,7 @@ int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, Sor
     o.gate = o.counters + kCtrGate;
     o.stray_count = o.counters + kCtrStrays;
     o.stray_list = o.idx[0];
-    o.rec_scratch = b + L.keys0;                         // keys0, keys1, idx0, idx1: 16 N bytes in a row
+    o.rec_scratch = b + L.keys0;                         // keys0, keys1, idx0, idx1, pkey, rec_extra: 32 N bytes in a row
     o.zero_begin = b + L.zero_begin;
     o.zero_bytes = L.zero_end - L.zero_begin;
     o.racc = (double*)(b + L.racc);
@@ -1039,7 +1048,7 @@ static int sort_impl(const pic_grid_t& g, const pic_particles_t& in, pic_particl
     if (rc != PIC_OK) return rc;
     const int64_t n = in.n;
     if (n > 0 && reorder) {
-        // most particles stay where they are: gather value by value; most of them move (first sort): 16-byte records
+        // most particles stay where they are: gather value by value; most of them move (first sort): 32-byte records
         if ((rc = launch_reorder(g, in, out, perm, ws.gate, 0u, st)) != PIC_OK) return rc;
         return launch_reorder_records(g, in, out, perm, ws.rec_scratch, ws.gate, 1u, st);
     }
