@@ -225,6 +225,23 @@ def sort_buckets(g: Grid, x, v, w, bucket):
     return xo, vo, wo, perm, off
 
 
+def sort_buckets_inplace(g: Grid, x, v, w, bucket):
+    """Alg. 2 (sort for pre-ordered particles, in place, only misplaced particles move)
+    -> (x, v, w copies after the sort, bucket_offsets[B+1] int32, number of particles moved)."""
+    n = w.shape[0]
+    _chk(g, list(x) + list(v) + [w], n)
+    xo = [a.copy() for a in x]
+    vo = [a.copy() for a in v]
+    wo = w.copy()
+    off = np.empty(bucket_count(g, bucket) + 1, np.int32)
+    moved = ctypes.c_int64(0)
+    cg = g.c()
+    _rc(_load().pic_ref_sort_buckets_inplace(ctypes.byref(cg), _bucket3(g, bucket), ctypes.c_int64(n), _ptrs(xo), _ptrs(vo),
+                                             ctypes.c_void_p(wo.ctypes.data), ctypes.c_void_p(off.ctypes.data),
+                                             ctypes.byref(moved)))
+    return xo, vo, wo, off, int(moved.value)
+
+
 def deposit(g: Grid, x, w, allpairs: bool = False) -> np.ndarray:
     """rho[C] in float64, x fastest."""
     n = w.shape[0]

@@ -320,6 +320,77 @@ int pic_ref_sort_buckets(const pic_ref_grid *g, const int32_t bucket[3], int64_t
 }
 
 /* ---------------------------------------------------------------------------
+ * NEXT-1. "Bucketsort for pre-ordered particles, contiguous datastructure" (Alg. 2; text
+ * PAPER.md:190-196): the sort the paper prefers ("for the rest of this paper this sorting algorithm is
+ * considered").  IN PLACE; only the misplaced particles move.  Steps, in the listing's order:
+ *   l.1-5   bucket_sizes = histogram of the keys, bucket_offsets = prefix sum
+ *   l.6-10  bucket_num[ip] = the bucket whose region [offsets[b], offsets[b+1]) holds array position ip
+ *   l.13-20 a particle is misplaced if bucket_num[ip] != key(ip); counts per bucket, offsets of the buffers
+ *   l.21-30 misplaced particles go to particles_buffer (grouped by TARGET bucket), their positions to holes_buffer
+ *           (grouped by SOURCE bucket = region)
+ *   l.31-35 the particles of the buffer are put into the holes of their target bucket
+ * The paper takes buffer slots with atomic counters, so which incoming particle lands in which hole of its bucket is
+ * arbitrary.  Reading (R24): slots in ascending array position on both sides -- the holes of a region in
+ * ascending position, the incoming particles of a bucket in ascending source position -- which makes the result
+ * unique.  Region b has as many holes as there are misplaced particles with key b (both equal bucket_sizes[b] minus
+ * the particles of key b already inside the region), so hole i of the whole array (ascending) receives misplaced
+ * particle i of the list sorted stably by key.  Not a stable sort: particles already in their region do not move.
+ * *moved = number of misplaced particles.  bucket = (1,1,1): cells.
+ * ------------------------------------------------------------------------- */
+int pic_ref_sort_buckets_inplace(const pic_ref_grid *g, const int32_t bucket[3], int64_t n,
+                                 void *const x[3], void *const v[3], void *w,
+                                 int32_t *bucket_offsets, int64_t *moved)
+{
+    if (!grid_ok(g) || !bucket_ok(g, bucket) || n < 0 || n > 2147483647LL) return REF_BAD_ARG;
+    int64_t B = pic_ref_bucket_count(g, bucket);
+    size_t s = g->dtype ? 8 : 4;
+    int A = 2 * g->dim + 1;
+    int32_t *key = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+    int32_t *bucket_num = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+    int32_t *buffer_sizes = (int32_t *)calloc((size_t)(B + 1), sizeof(int32_t));
+    int32_t *buffer_offsets = (int32_t *)calloc((size_t)(B + 1), sizeof(int32_t));
+    int32_t *counter_pbuffer = (int32_t *)calloc((size_t)(B + 1), sizeof(int32_t));
+    if (!key || !bucket_num || !buffer_sizes || !buffer_offsets || !counter_pbuffer) return REF_BAD_ARG;
+    void *arr[7];
+    for (int c = 0; c < g->dim; ++c) { arr[c] = x[c]; arr[g->dim + c] = v[c]; }
+    arr[2 * g->dim] = w;
+
+    for (int64_t k = 0; k <= B; ++k) bucket_offsets[k] = 0;                 /* l.1-5 */
+    for (int64_t i = 0; i < n; ++i) {
+        key[i] = bucket_key(g, bucket, (const void *const *)x, i);
+        bucket_offsets[key[i] + 1] += 1;
+    }
+    for (int64_t k = 0; k < B; ++k) bucket_offsets[k + 1] += bucket_offsets[k];
+    for (int64_t b = 0; b < B; ++b)                                          /* l.6-10 */
+        for (int64_t ic = bucket_offsets[b]; ic < bucket_offsets[b + 1]; ++ic) bucket_num[ic] = (int32_t)b;
+    int64_t M = 0;                                                           /* l.13-17: incoming per TARGET bucket */
+    for (int64_t ip = 0; ip < n; ++ip)
+        if (bucket_num[ip] != key[ip]) { buffer_sizes[key[ip]] += 1; ++M; }
+    for (int64_t b = 0; b < B; ++b) buffer_offsets[b + 1] = buffer_offsets[b] + buffer_sizes[b];   /* l.18-20 */
+    char *particles_buffer = (char *)malloc((size_t)(M > 0 ? M : 1) * (size_t)A * s);
+    int32_t *holes_buffer = (int32_t *)malloc(sizeof(int32_t) * (size_t)(M > 0 ? M : 1));
+    if (!particles_buffer || !holes_buffer) return REF_BAD_ARG;
+    int64_t nholes = 0;
+    for (int64_t ip = 0; ip < n; ++ip) {                                     /* l.21-30, ascending position */
+        int32_t source_bucket = bucket_num[ip], target_bucket = key[ip];
+        if (target_bucket != source_bucket) {
+            int64_t lcpbuffer = counter_pbuffer[target_bucket]++;
+            int64_t slot = lcpbuffer + buffer_offsets[target_bucket];
+            for (int a = 0; a < A; ++a)
+                memcpy(particles_buffer + ((size_t)slot * (size_t)A + (size_t)a) * s, (const char *)arr[a] + s * (size_t)ip, s);
+            holes_buffer[nholes++] = (int32_t)ip;          /* regions are ordered by position: grouped by source bucket */
+        }
+    }
+    for (int64_t i = 0; i < M; ++i)                                          /* l.31-35 */
+        for (int a = 0; a < A; ++a)
+            memcpy((char *)arr[a] + s * (size_t)holes_buffer[i], particles_buffer + ((size_t)i * (size_t)A + (size_t)a) * s, s);
+    if (moved) *moved = M;
+    free(key); free(bucket_num); free(buffer_sizes); free(buffer_offsets); free(counter_pbuffer);
+    free(particles_buffer); free(holes_buffer);
+    return REF_OK;
+}
+
+/* ---------------------------------------------------------------------------
  * O3 / a5. Charge deposit (setrho, threads-on-particles form without the threads:
  * PAPER.md:292-294 section 3.3.4; the 8 products of PAPER.md:509-519 for p = 1).
  *   rho[j] = h^-d sum_i w_i prod_c W_p(x_ic/h_c - j_c)   on the periodic grid.
