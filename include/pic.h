@@ -221,8 +221,24 @@ int pic_step(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t 
  *   CELL key (short inside a bucket, where the source order is kept), particles alone in their run going the
  *   threads-on-particles way (setrho 3.3.4).  The result is exact for every bucket size; one cell per
  *   bucket is by far the fastest on this hardware (the sweep is in profiles/ and DESIGN.md).
+ *
+ * pic_sort_buckets_inplace: the paper's preferred sort, "Bucketsort for pre-ordered particles, contiguous datastructure"
+ *   (Alg. 2; text PAPER.md:190-196; "for the rest of this paper this sorting algorithm is
+ *   considered"): IN PLACE, and only the misplaced particles move.  bucket_offsets
+ *   (OUT only) = prefix sum of the key histogram; a particle is misplaced if its array position lies outside the region
+ *   [offsets[key], offsets[key+1]) of its own key (l.6-17 of the listing); misplaced particles are copied to a buffer
+ *   grouped by target bucket, their positions are the holes, grouped by region; buffer entry i goes into hole i
+ *   (l.21-35).  The paper hands out buffer slots with atomic counters; here slots go in ascending array position on both
+ *   sides (R24), so the result is unique.  NOT stable: particles already inside their region stay where they are.
+ *   *moved (device int32, may be NULL) = number of misplaced particles.  ws: pic_sort_buckets_inplace_bytes() =
+ *   pic_workspace_bytes() + all attributes of n particles (the particles_buffer at its largest).
+ *   With one cell per bucket and many cells most particles count as misplaced after a single step, because every cell
+ *   boundary shifts by the net flux of all cells below it; the sort pays off for large buckets.
  */
 int pic_bucket_count(const pic_grid_t *grid, const int32_t bucket[3] /* host */, int64_t *count /* host, out */);
+int pic_sort_buckets_inplace_bytes(const pic_grid_t *grid, int64_t n, size_t *bytes /* host, out */);
+int pic_sort_buckets_inplace(const pic_grid_t *grid, const int32_t bucket[3] /* host */, pic_particles_t *p,
+                             int32_t *bucket_offsets, int32_t *moved, void *ws, size_t ws_bytes, void *stream);
 int pic_sort_buckets(const pic_grid_t *grid, const int32_t bucket[3] /* host */, const pic_particles_t *in,
                      pic_particles_t *out, int32_t *perm, int32_t *bucket_offsets, void *ws, size_t ws_bytes,
                      void *stream);

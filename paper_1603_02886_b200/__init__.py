@@ -22,7 +22,7 @@ PIC_SORT, PIC_SORT_CHAINED = 1, 3
 
 EXPORTS = ("pic_workspace_bytes", "pic_sort", "pic_deposit", "pic_push", "pic_step",
            "pic_step_host_bytes", "pic_step_host", "pic_step_fields_host_bytes", "pic_step_fields_host",
-           "pic_bucket_count", "pic_sort_buckets", "pic_step_buckets", "pic_deposit_nodes", "pic_deposit_replicated_bytes", "pic_deposit_replicated",
+           "pic_bucket_count", "pic_sort_buckets", "pic_step_buckets", "pic_sort_buckets_inplace_bytes", "pic_sort_buckets_inplace", "pic_deposit_nodes", "pic_deposit_replicated_bytes", "pic_deposit_replicated",
            "pic_field_solve_bytes", "pic_field_solve", "pic_step_selfconsistent_bytes", "pic_step_selfconsistent",
            "pic_last_launch_count", "pic_set_phase_events",
            "pic_strerror")
@@ -80,6 +80,8 @@ def lib():
         B3 = ctypes.POINTER(ctypes.c_int32)
         L.pic_bucket_count.argtypes = [G, B3, ctypes.POINTER(i64)]
         L.pic_sort_buckets.argtypes = [G, B3, P, P, vp, vp, vp, sz, vp]
+        L.pic_sort_buckets_inplace_bytes.argtypes = [G, i64, ctypes.POINTER(sz)]
+        L.pic_sort_buckets_inplace.argtypes = [G, B3, P, vp, vp, vp, sz, vp]
         L.pic_step_buckets.argtypes = [G, B3, P, P, vp, vp, vp, E3, dbl, dbl, vp, sz, vp]
         L.pic_deposit_nodes.argtypes = [G, P, vp, vp, vp, sz, vp]
         L.pic_deposit_replicated_bytes.argtypes = [G, i64, ctypes.POINTER(sz)]
@@ -249,6 +251,24 @@ def pic_sort_buckets(g: Grid, bucket, x_in, v_in, w_in, x_out, v_out, w_out, per
     _check(lib().pic_sort_buckets(ctypes.byref(cg), _bucket3(g, bucket), ctypes.byref(pi), ctypes.byref(po), _ptr(perm),
                                   _ptr(bucket_offsets), _ptr(ws), ws.numel() * ws.element_size(), _stream(stream)),
            "pic_sort_buckets")
+
+
+def pic_sort_buckets_inplace_bytes(g: Grid, n: int) -> int:
+    cg, out = g.c(), ctypes.c_size_t(0)
+    _check(lib().pic_sort_buckets_inplace_bytes(ctypes.byref(cg), n, ctypes.byref(out)), "pic_sort_buckets_inplace_bytes")
+    return int(out.value)
+
+
+def pic_sort_buckets_inplace(g: Grid, bucket, x, v, w, bucket_offsets, moved, ws, stream=None):
+    """Alg. 2: sort x, v, w IN PLACE by bucket key, moving only the misplaced particles; bucket_offsets[B+1] out;
+    moved: int32 CUDA tensor of one element (or None)."""
+    n = w.numel()
+    _dev_check(g, list(x) + list(v) + [w], n)
+    cg = g.c()
+    p = _particles(g, x, v, w, n)
+    _check(lib().pic_sort_buckets_inplace(ctypes.byref(cg), _bucket3(g, bucket), ctypes.byref(p), _ptr(bucket_offsets),
+                                          _ptr(moved), _ptr(ws), ws.numel() * ws.element_size(), _stream(stream)),
+           "pic_sort_buckets_inplace")
 
 
 def pic_step_buckets(g: Grid, bucket, x_in, v_in, w_in, x_out, v_out, w_out, perm, bucket_offsets, rho, E, dt: float,

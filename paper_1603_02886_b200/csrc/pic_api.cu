@@ -321,6 +321,33 @@ int pic_sort_buckets(const pic_grid_t* grid, const int32_t bucket[3], const pic_
     return launch_sort(*grid, *in, o, perm, bucket_offsets, sws, true, false, (cudaStream_t)stream);
 }
 
+int pic_sort_buckets_inplace_bytes(const pic_grid_t* grid, int64_t n, size_t* bytes)
+{
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if (!bytes || n < 0 || n >= ((int64_t)1 << 30)) return PIC_ERR_INVALID_ARG;
+    const size_t s = grid->dtype == PIC_F64 ? 8 : 4;
+    *bytes = sort_ws_bytes(*grid, n) + align256(s * (size_t)(2 * grid->dim + 1) * (size_t)(n > 0 ? n : 1));
+    return PIC_OK;
+}
+
+int pic_sort_buckets_inplace(const pic_grid_t* grid, const int32_t bucket[3], pic_particles_t* p, int32_t* bucket_offsets,
+                             int32_t* moved, void* ws, size_t ws_bytes, void* stream)
+{
+    g_launches = 0;
+    int rc = check_grid(grid);
+    if (rc != PIC_OK) return rc;
+    if ((rc = check_bucket(*grid, bucket)) != PIC_OK) return rc;
+    if ((rc = check_particles(*grid, p, true, true)) != PIC_OK) return rc;
+    if (!aligned16(bucket_offsets) || !aligned16(ws)) return PIC_ERR_INVALID_ARG;
+    const size_t s = grid->dtype == PIC_F64 ? 8 : 4;
+    const size_t sb = sort_ws_bytes(*grid, p->n);
+    if (ws_bytes < sb + align256(s * (size_t)(2 * grid->dim + 1) * (size_t)(p->n > 0 ? p->n : 1))) return PIC_ERR_WORKSPACE;
+    SortWs sws;
+    if ((rc = carve_sort_ws(*grid, p->n, ws, sb, sws, bucket)) != PIC_OK) return rc;
+    return launch_sort_inplace(*grid, *p, bucket_offsets, sws, (char*)ws + sb, moved, (cudaStream_t)stream);
+}
+
 int pic_step_buckets(const pic_grid_t* grid, const int32_t bucket[3], const pic_particles_t* in, pic_particles_t* out,
                      int32_t* perm, int32_t* bucket_offsets, void* rho, const void* const E[3], double dt, double qm,
                      void* ws, size_t ws_bytes, void* stream)

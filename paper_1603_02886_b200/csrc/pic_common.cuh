@@ -264,6 +264,9 @@ int carve_sort_ws(const pic_grid_t& g, int64_t n, void* ws, size_t ws_bytes, Sor
 // workspace's ChainSig): keys, histograms and the stayer/mover split are then the ones that step emitted.
 int launch_sort(const pic_grid_t& g, const pic_particles_t& in, pic_particles_t& out, int32_t* perm,
                 int32_t* cell_offsets, const SortWs& ws, bool reorder, bool chained, cudaStream_t st);
+// Alg. 2: sort in place by moving only the misplaced particles (ws carved with the bucket shape; buffer: A arrays of n)
+int launch_sort_inplace(const pic_grid_t& g, const pic_particles_t& p, int32_t* offsets, const SortWs& ws, void* buffer,
+                        int32_t* moved, cudaStream_t st);
 int launch_chain_commit(const pic_grid_t& g, const pic_particles_t& out, const SortWs& ws, cudaStream_t st);
 int launch_deposit(const pic_grid_t& g, const pic_particles_t& p, int order_state,
                    const int32_t* cell_offsets, void* rho, double* racc, cudaStream_t st);

@@ -976,8 +976,10 @@ ChainSig chain_sig_of(const pic_grid_t& g, const pic_particles_t& p)
 
 template <typename T, int D>
 static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_t* perm, int32_t* cell_offsets,
-                          const SortWs& ws, bool chained, cudaStream_t st)
+                          const SortWs& ws, bool chained, cudaStream_t st, uint32_t* holes = nullptr, int* sorted_src = nullptr)
 {
+    // holes != NULL (launch_sort_inplace): the movers' positions, in position order, are copied there before the radix
+    // passes; every pass keeps its (key, position) lists (*sorted_src = the buffer that ends up sorted); perm is not written
     const int64_t n = in.n;
     const int C = (int)ws.nkeys;                      // cells, or buckets (pic_sort_buckets)
     mark_phase(PIC_PHASE_BEGIN, st);
@@ -1002,6 +1004,7 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
                                                                 ws.mprefix, ws.tile_base, (int)ws.stage_tiles, n, ws.counters,
                                                                 ws.chain_sig);
         count_launch(5);
+        if (holes) PIC_CUDA_OK(cudaMemcpyAsync(holes, ws.idx[0], sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToDevice, st));
     } else {
         PIC_CUDA_OK(cudaMemsetAsync(ws.hist_begin, 0, ws.hist_bytes, st));
     }
@@ -1021,7 +1024,7 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
         int src = 0;
         const PermP pp{cell_offsets, ws.mover_off, ws.old_off, perm};
         for (int q = 0; q < ws.passes; ++q) {
-            auto kern = (q == ws.passes - 1) ? k_radix_pass<true> : k_radix_pass<false>;
+            auto kern = (!holes && q == ws.passes - 1) ? k_radix_pass<true> : k_radix_pass<false>;
             kern<<<(unsigned)ws.radix_tiles, kRadixThreads, 0, st>>>(
                 ws.keys[src], ws.idx[src], ws.keys[src ^ 1], ws.idx[src ^ 1], ws.counters, q * ws.bits_per_pass,
                 (1u << ws.bits_per_pass) - 1u, ws.digit_hist + q * kRadix, ws.counters + kCtrRadix + q,
@@ -1030,6 +1033,11 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
             src ^= 1;
         }
         mark_phase(PIC_PHASE_RADIX, st);
+        if (sorted_src) *sorted_src = src;
+        if (holes) {
+            mark_phase(PIC_PHASE_REORDER, st);
+            return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+        }
         k_cell_base<<<(unsigned)((C + 255) / 256), 256, 0, st>>>(cell_offsets, ws.old_off, ws.mover_lo, ws.mask, ws.mprefix,
                                                                  ws.cell_base, C, ws.counters);
         k_perm_stayers<<<(unsigned)((n + 256 * kStayIPT - 1) / (256 * kStayIPT)), 256, 0, st>>>(
@@ -1053,6 +1061,108 @@ static int sort_impl(const pic_grid_t& g, const pic_particles_t& in, pic_particl
         return launch_reorder_records(g, in, out, perm, ws.rec_scratch, ws.gate, 1u, st);
     }
     return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+}
+
+// ----------------------------------------------------------------------------- Alg. 2: in place, only misplaced particles move
+// "Bucketsort for pre-ordered particles, contiguous datastructure" (Alg. 2; 190-196; the sort the
+// paper prefers).  bucket_sizes and bucket_offsets first (l.1-5: k_keys_hist, k_scan_cells); a particle
+// is MISPLACED if its position lies outside the region [offsets[key], offsets[key+1]) of its own key (l.6-17:
+// bucket_num[ip] != key) -- which is this file's stayer/mover split with the NEW offsets as the hint, so k_classify and
+// the movers' radix sort do l.13-30: the movers in position order are the holes_buffer (regions are ordered by
+// position), the movers sorted stably by key are the particles_buffer (grouped by target bucket); l.31-35: buffer
+// entry i goes into hole i (reading R24: slots in ascending position; the paper's atomic counters leave it open).
+template <typename T, int D, bool BK>
+__global__ void __launch_bounds__(256) k_keys_hist(PartP<T> p, GridP<T> g, int n, int32_t* __restrict__ count)
+{
+    const int lane = threadIdx.x & 31;
+    for (int base = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; base < n; base += gridDim.x * blockDim.x) {
+        const int i = base + lane;
+        int key = -1;
+        if (i < n) {
+            int cell[3] = {0, 0, 0};
+#pragma unroll
+            for (int c = 0; c < D; ++c) cell[c] = cell_index(grid_coord(p.x[c][i], g.h[c], g.inv_h[c], g.hmul), g.n[c]);
+            key = sort_key<T, D, BK>(g, cell);
+        }
+        const unsigned peers = __match_any_sync(0xFFFFFFFFu, key);       // one atomic per distinct key of the warp
+        if (key >= 0 && lane == __ffs(peers) - 1) atomicAdd(&count[key], __popc(peers));
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_alg2_gather(RecPtrs<T> a, T* __restrict__ buf, int64_t stride, const uint32_t* __restrict__ sorted_idx,
+                                                     const uint32_t* __restrict__ counters)
+{
+    const int64_t m = counters[kCtrMovers];
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += (int64_t)gridDim.x * blockDim.x) {
+        const uint32_t from = sorted_idx[i];
+#pragma unroll
+        for (int k = 0; k < 7; ++k)
+            if (a.s[k]) buf[k * stride + i] = a.s[k][from];
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_alg2_scatter(RecPtrs<T> a, const T* __restrict__ buf, int64_t stride, const uint32_t* __restrict__ holes,
+                                                      const uint32_t* __restrict__ counters, int32_t* __restrict__ moved)
+{
+    const int64_t m = counters[kCtrMovers];
+    if (moved && blockIdx.x == 0 && threadIdx.x == 0) *moved = (int32_t)m;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += (int64_t)gridDim.x * blockDim.x) {
+        const uint32_t to = holes[i];
+#pragma unroll
+        for (int k = 0; k < 7; ++k)
+            if (a.d[k]) a.d[k][to] = buf[k * stride + i];
+    }
+}
+
+template <typename T, int D>
+static int sort_inplace_impl(const pic_grid_t& g, const pic_particles_t& p, int32_t* offsets, const SortWs& ws, void* buffer,
+                             int32_t* moved, cudaStream_t st)
+{
+    const int64_t n = p.n;
+    const int C = (int)ws.nkeys;
+    // l.1-5: histogram and prefix sum -> the offsets, which are then the hint of the split below
+    PIC_CUDA_OK(cudaMemsetAsync(ws.zero_begin, 0, ws.zero_bytes, st));
+    PIC_CUDA_OK(cudaMemsetAsync(ws.hist_begin, 0, ws.hist_bytes, st));
+    if (n > 0) {
+        const int64_t want_blocks = (n + 255) / 256, cap = (int64_t)sm_count() * 16;
+        auto kh = ws.bucket ? k_keys_hist<T, D, true> : k_keys_hist<T, D, false>;
+        kh<<<(unsigned)(want_blocks < cap ? want_blocks : cap), 256, 0, st>>>(make_partp<T>(p), make_gridp<T>(g, ws.bucket), (int)n, ws.cell_count);
+        count_launch();
+    }
+    k_scan_cells<<<(unsigned)ws.scan_tiles, kScanThreads, 0, st>>>(ws.cell_count, offsets, C, ws.scan_status, ws.counters + kCtrScanA,
+                                                                    nullptr, 0, 0);
+    count_launch();
+    // l.6-30: misplaced particles (position outside the region of their key), in position order and sorted by key
+    int src = 0;
+    int rc = sort_keys_perm<T, D>(g, p, nullptr, offsets, ws, false, st, ws.pkey, &src);
+    if (rc != PIC_OK) return rc;
+    if (n > 0) {                                       // l.31-35 through the particles_buffer
+        RecPtrs<T> rp;
+        int A = 0;
+        for (int k = 0; k < 8; ++k) { rp.s[k] = nullptr; rp.d[k] = nullptr; }
+        for (int c = 0; c < g.dim; ++c) { rp.s[A] = (const T*)p.x[c]; rp.d[A++] = (T*)p.x[c]; }
+        for (int c = 0; c < g.dim; ++c) { rp.s[A] = (const T*)p.v[c]; rp.d[A++] = (T*)p.v[c]; }
+        rp.s[A] = (const T*)p.w; rp.d[A++] = (T*)p.w;
+        const unsigned blocks = (unsigned)(sm_count() * 8);
+        k_alg2_gather<T><<<blocks, 256, 0, st>>>(rp, (T*)buffer, n, ws.idx[src], ws.counters);
+        k_alg2_scatter<T><<<blocks, 256, 0, st>>>(rp, (const T*)buffer, n, ws.pkey, ws.counters, moved);
+        count_launch(2);
+    } else if (moved) {
+        PIC_CUDA_OK(cudaMemsetAsync(moved, 0, sizeof(int32_t), st));
+    }
+    return cudaPeekAtLastError() == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+}
+
+int launch_sort_inplace(const pic_grid_t& g, const pic_particles_t& p, int32_t* offsets, const SortWs& ws, void* buffer,
+                        int32_t* moved, cudaStream_t st)
+{
+    if (g.dtype == PIC_F32)
+        return g.dim == 2 ? sort_inplace_impl<float, 2>(g, p, offsets, ws, buffer, moved, st)
+                          : sort_inplace_impl<float, 3>(g, p, offsets, ws, buffer, moved, st);
+    return g.dim == 2 ? sort_inplace_impl<double, 2>(g, p, offsets, ws, buffer, moved, st)
+                      : sort_inplace_impl<double, 3>(g, p, offsets, ws, buffer, moved, st);
 }
 
 // the next call may chain on to the step that has just been enqueued on `out`

@@ -196,3 +196,60 @@ def test_unit_buckets_equal_the_cell_step():
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
     for a, b in zip(outs[0][2], outs[1][2]):
         assert np.array_equal(a, b)
+
+
+# ---- pic_sort_buckets_inplace: Alg. 2, only misplaced particles move ------------------------
+INPLACE_CASES = [
+    ("cfg2", 200_003, (64, 64), (8, 8), True), ("cfg2", 200_003, (64, 64), (1, 1), True), ("cfg2", 150_001, (48, 40), (5, 7), True),
+    ("cfg3", 150_001, (32, 32, 32), (4, 4, 4), True), ("cfg3", 150_001, (32, 32, 32), (1, 1, 1), True),
+    ("cfg3", 150_001, (32, 32, 32), (8, 8, 8), False),        # random order: nearly everything is misplaced
+    ("cfg4", 300_007, (32, 32, 32), (4, 4, 4), True), ("cfg5", 8 * 16 ** 3 + 5, (16, 16, 16), (4, 2, 1), True),
+    ("cfg1", 100_000, (64, 64), (32, 16), True), ("cfg3", 60_000, (16, 16, 16), (16, 16, 16), False),   # one bucket: nothing moves
+]
+
+
+@pytest.mark.parametrize("name,N,n,bucket,presort", INPLACE_CASES)
+def test_sort_buckets_inplace_bit_exact(name, N, n, bucket, presort):
+    """The whole particle arrays, the offsets and the number of moved particles equal the oracle's Alg. 2 bit for bit
+    (slots in ascending position make the result unique, R24)."""
+    O, B = _mods()
+    cfg = _cfg(name, N, n=n)
+    wl = W.make_workload(cfg)
+    go, gb = O.grid_of(cfg), B.grid_of(cfg)
+    x, v, w = wl.x, wl.v, wl.w
+    if presort:
+        x, v, w, _, _ = O.sort_buckets(go, x, v, w, bucket)
+        x, v = O.push(go, x, v, wl.E, cfg.dt, cfg.qm)
+    rx, rv, rw, roff, rmoved = O.sort_buckets_inplace(go, x, v, w, bucket)
+    xd, vd, wd = to_dev(x), to_dev(v), to_dev([w])[0]
+    nb = B.pic_bucket_count(gb, bucket)
+    off = torch.full((nb + 4,), -7, dtype=torch.int32, device="cuda")
+    moved = torch.full((4,), -1, dtype=torch.int32, device="cuda")
+    ws = torch.full((B.pic_sort_buckets_inplace_bytes(gb, N),), 0x5C, dtype=torch.uint8, device="cuda")
+    B.pic_sort_buckets_inplace(gb, bucket, xd, vd, wd, off, moved, ws)
+    torch.cuda.synchronize()
+    assert int(moved[0].item()) == rmoved
+    assert np.array_equal(off[: nb + 1].cpu().numpy(), roff)
+    for c in range(cfg.dim):
+        assert np.array_equal(xd[c].cpu().numpy(), rx[c]) and np.array_equal(vd[c].cpu().numpy(), rv[c])
+    assert np.array_equal(wd.cpu().numpy(), rw)
+    if nb == 1:
+        assert rmoved == 0
+
+
+@pytest.mark.parametrize("N", [0, 1, 33, 4097])
+def test_sort_buckets_inplace_edge_sizes(N):
+    O, B = _mods()
+    cfg = _cfg("cfg2", N, n=(16, 16))
+    wl = W.make_workload(cfg)
+    rx, rv, rw, roff, rmoved = O.sort_buckets_inplace(O.grid_of(cfg), wl.x, wl.v, wl.w, (4, 4))
+    gb = B.grid_of(cfg)
+    xd, vd, wd = to_dev(wl.x), to_dev(wl.v), to_dev([wl.w])[0]
+    off = torch.zeros(16 + 4, dtype=torch.int32, device="cuda")
+    moved = torch.zeros(4, dtype=torch.int32, device="cuda")
+    ws = torch.empty(B.pic_sort_buckets_inplace_bytes(gb, N), dtype=torch.uint8, device="cuda")
+    B.pic_sort_buckets_inplace(gb, (4, 4), xd, vd, wd, off, moved, ws)
+    torch.cuda.synchronize()
+    assert int(moved[0].item()) == rmoved and np.array_equal(off[:17].cpu().numpy(), roff)
+    if N:
+        assert np.array_equal(xd[0].cpu().numpy(), rx[0]) and np.array_equal(wd.cpu().numpy(), rw)
