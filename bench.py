@@ -212,6 +212,9 @@ def main():
                     help="replay the steps from CUDA graphs (small, launch-bound problems; no per-phase times)")
     ap.add_argument("--closed-loop", action="store_true",
                     help="the timed step is pic_step_selfconsistent: sort, deposit, Poisson solve, accel, push (not the headline)")
+    ap.add_argument("--sort-compare", action="store_true",
+                    help="with --bucket: also time pic_sort_buckets (stable, out of place) against pic_sort_buckets_inplace "
+                         "(Alg. 2) on the pre-ordered particles of the run")
     ap.add_argument("--deposit-compare", action="store_true",
                     help="also time pic_deposit (sorted / never sorted) and pic_deposit_nodes on this workload")
     ap.add_argument("--ref-particles", type=int, default=2_000_000)
@@ -420,6 +423,10 @@ def main():
     if (args.config == "cfg5" or args.deposit_compare) and world == 1 and bucket is None:
         deposit_compare = run_deposit_compare(B, torch, cfg, g, wl, st, dev, nodes=args.deposit_compare)
 
+    sort_compare = None
+    if args.sort_compare and bucket is not None and world == 1:
+        sort_compare = run_sort_compare(B, torch, cfg, g, st, bucket, dev)
+
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
         cpu_baseline = run_cpu_baseline(cfg, args.cpu_particles)
@@ -440,6 +447,8 @@ def main():
     if bucket is not None:
         line["config"]["bucket"] = list(bucket)
         line["config"]["workload"] += ", buckets of %s cells (pic_step_buckets)" % "x".join(map(str, bucket))
+    if sort_compare:
+        line["sort_ms"] = sort_compare
     if graph_line:
         line["cuda_graph"] = graph_line
     if deposit_compare:
@@ -554,6 +563,39 @@ def run_deposit_compare(B, torch, cfg, g, wl, st, dev, reps=5, nodes=False):
         out["nodes_deterministic"] = t_nodes
         out["replicated_deterministic"] = t_repl
     return out
+
+
+def run_sort_compare(B, torch, cfg, g, st, bucket, dev, reps=3):
+    """ms per sort of the run's pre-ordered particles (bucket order of the last step, advanced by one push): the stable
+    out-of-place sort with the previous offsets as hint, against Alg. 2 in place (only misplaced particles move)."""
+    a = st.cur
+    n = cfg.N
+    tmp = dict(x=[torch.empty_like(t) for t in a["x"]], v=[torch.empty_like(t) for t in a["v"]], w=torch.empty_like(a["w"]))
+    nb = B.pic_bucket_count(g, bucket)
+    off = torch.empty(nb + 4, dtype=torch.int32, device=dev)
+    moved = torch.zeros(4, dtype=torch.int32, device=dev)
+    ws2 = torch.empty(B.pic_sort_buckets_inplace_bytes(g, n), dtype=torch.uint8, device=dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_stable, t_inplace = [], []
+    for r in range(reps + 1):
+        off[: nb + 1].copy_(st.cell_offsets[: nb + 1])                 # the hint: offsets of the order the particles are in
+        e0.record()
+        B.pic_sort_buckets(g, bucket, a["x"], a["v"], a["w"], tmp["x"], tmp["v"], tmp["w"], st.perm, off, st.ws)
+        e1.record()
+        torch.cuda.synchronize()
+        if r:
+            t_stable.append(e0.elapsed_time(e1))
+        for c in range(cfg.dim):
+            tmp["x"][c].copy_(a["x"][c]); tmp["v"][c].copy_(a["v"][c])
+        tmp["w"].copy_(a["w"])
+        e0.record()
+        B.pic_sort_buckets_inplace(g, bucket, tmp["x"], tmp["v"], tmp["w"], off, moved, ws2)
+        e1.record()
+        torch.cuda.synchronize()
+        if r:
+            t_inplace.append(e0.elapsed_time(e1))
+    return {"stable_out_of_place": sum(t_stable) / reps, "alg2_in_place": sum(t_inplace) / reps,
+            "misplaced_fraction": int(moved[0].item()) / max(n, 1), "unit": "ms per sort of the pre-ordered particles"}
 
 
 def run_cpu_baseline(cfg, sample):
