@@ -52,7 +52,8 @@ typedef enum {
     PIC_ERR_INVALID_ARG = -1,   /* null/misaligned pointer, bad dim/order/n/h/N */
     PIC_ERR_UNSUPPORTED = -2,   /* valid request this build has no kernel for */
     PIC_ERR_WORKSPACE = -3,     /* ws_bytes < pic_workspace_bytes() */
-    PIC_ERR_CUDA = -4           /* launch failure; see cudaGetLastError() */
+    PIC_ERR_CUDA = -4,          /* launch failure; see cudaGetLastError() */
+    PIC_ERR_TOO_LARGE = -5      /* pic_deposit_static: the grid has more than PIC_DEPOSIT_STATIC_MAX_NODES nodes */
 } pic_status_t;
 
 /* How the particle array handed to pic_deposit / pic_push is ordered. */
@@ -122,6 +123,37 @@ int pic_sort(const pic_grid_t *grid, const pic_particles_t *in, pic_particles_t 
  */
 int pic_deposit(const pic_grid_t *grid, const pic_particles_t *p, int order_state,
                 const int32_t *cell_offsets, void *rho, void *ws, size_t ws_bytes, void *stream);
+
+/*
+ * pic_deposit_static -- pic_deposit for callers that cannot allocate device memory: no workspace argument.
+ *
+ * Why it exists.  On an fp32 grid pic_deposit sums in a double-precision copy of the grid (rounded into rho once at the
+ * end) and takes that copy from a caller-allocated workspace.  A caller that is only handed its input and output
+ * buffers has nowhere to get one: a plug-in inside an application that owns the device heap, code on a latency budget
+ * where cudaMalloc / cudaFree are ruled out because they may synchronise the device, or a process that starts after all
+ * GPU memory went to pools.  For them the double grid is a fixed-size array INSIDE the library: every GPU that loads the
+ * library carries PIC_DEPOSIT_STATIC_MAX_NODES doubles (16 MiB) of it until the process exits, used or not.
+ *
+ * What it computes.  rho[C] (overwritten) exactly as pic_deposit(grid, p, PIC_ORDER_UNSORTED, ...) does: the paper's
+ * "threads on particles" deposit with atomic additions (setrho 3.3.4; formula and R2/R10 as for
+ * pic_deposit), correct for any particle order; the two agree to the rounding of the double sums.  Only x[c] (c < dim)
+ * and w of p are read.
+ *
+ * Limits and rules.
+ *  - dtype must be PIC_F32.  PIC_F64 returns PIC_ERR_UNSUPPORTED: an fp64 grid sums in rho itself, so plain pic_deposit
+ *    with ws = NULL already allocates nothing.
+ *  - prod n <= PIC_DEPOSIT_STATIC_MAX_NODES (2^21 = a 128^3 grid), else PIC_ERR_TOO_LARGE and nothing is enqueued.
+ *  - The call itself never calls cudaMalloc, cudaFree or a library routine that allocates; it enqueues one memset and
+ *    two kernels on `stream`.
+ *  - The FIRST call on each device looks up that device's address of the array (cudaGetSymbolAddress, with the device
+ *    current; it may make the runtime load the library's code onto that device).  Make that first call during set-up,
+ *    before any stream capture is open, with the device that `stream` belongs to current -- as for every call.
+ *  - All calls on one device share the one array and find the previous call's sums in it; each call clears the part it
+ *    uses first, on its stream.  Two calls that can run at the same time on the GPU (different streams without an
+ *    ordering between them, or two host threads) RACE on the array and both get wrong densities.  Order them.
+ */
+#define PIC_DEPOSIT_STATIC_MAX_NODES (1 << 21)
+int pic_deposit_static(const pic_grid_t *grid, const pic_particles_t *p, void *rho, void *stream);
 
 /*
  * pic_deposit_nodes -- the same rho by the paper's COLLISION-FREE algorithm, "threads on splines" (setrho_splines,

@@ -23,6 +23,7 @@ PIC_SORT, PIC_SORT_CHAINED = 1, 3
 EXPORTS = ("pic_workspace_bytes", "pic_sort", "pic_deposit", "pic_push", "pic_step",
            "pic_step_host_bytes", "pic_step_host", "pic_step_fields_host_bytes", "pic_step_fields_host",
            "pic_bucket_count", "pic_sort_buckets", "pic_step_buckets", "pic_sort_buckets_inplace_bytes", "pic_sort_buckets_inplace", "pic_deposit_nodes", "pic_deposit_replicated_bytes", "pic_deposit_replicated",
+           "pic_deposit_static",
            "pic_field_solve_bytes", "pic_field_solve", "pic_step_selfconsistent_bytes", "pic_step_selfconsistent",
            "pic_last_launch_count", "pic_set_phase_events",
            "pic_strerror")
@@ -84,6 +85,7 @@ def lib():
         L.pic_sort_buckets_inplace.argtypes = [G, B3, P, vp, vp, vp, sz, vp]
         L.pic_step_buckets.argtypes = [G, B3, P, P, vp, vp, vp, E3, dbl, dbl, vp, sz, vp]
         L.pic_deposit_nodes.argtypes = [G, P, vp, vp, vp, sz, vp]
+        L.pic_deposit_static.argtypes = [G, P, vp, vp]
         L.pic_deposit_replicated_bytes.argtypes = [G, i64, ctypes.POINTER(sz)]
         L.pic_deposit_replicated.argtypes = [G, P, vp, vp, vp, sz, vp]
         L.pic_field_solve_bytes.argtypes = [G, ctypes.POINTER(sz)]
@@ -294,6 +296,24 @@ def pic_deposit(g: Grid, x, w, rho, order_state=PIC_ORDER_UNSORTED, cell_offsets
     wsb = ws.numel() * ws.element_size() if ws is not None else 0
     _check(lib().pic_deposit(ctypes.byref(cg), ctypes.byref(p), order_state, _ptr(cell_offsets), _ptr(rho),
                              _ptr(ws), wsb, _stream(stream)), "pic_deposit")
+
+
+PIC_DEPOSIT_STATIC_MAX_NODES = 1 << 21
+
+
+def pic_deposit_static(g: Grid, x, w, rho, stream=None):
+    """rho[C] (overwritten) as pic_deposit(..., PIC_ORDER_UNSORTED) computes it, WITHOUT a workspace: for callers that
+    may not allocate device memory (a plug-in that is only handed its buffers, code on a latency budget that rules out
+    cudaMalloc, a process whose GPU memory is all in pools).  The double-precision sums of the fp32 deposit live in a
+    16 MiB array inside the library.  fp32 grids of at most PIC_DEPOSIT_STATIC_MAX_NODES nodes; any particle order.
+    Calls share that array: do not let two of them overlap on the GPU.  The first call on a device does a one-time
+    address look-up and should be made before any stream capture (see include/pic.h)."""
+    n = w.numel()
+    _dev_check(g, list(x) + [w], n)
+    _dev_check(g, [rho], g.cells)
+    cg = g.c()
+    p = _particles(g, x, None, w, n)
+    _check(lib().pic_deposit_static(ctypes.byref(cg), ctypes.byref(p), _ptr(rho), _stream(stream)), "pic_deposit_static")
 
 
 def pic_deposit_nodes(g: Grid, x, w, rho, cell_offsets, ws, stream=None):

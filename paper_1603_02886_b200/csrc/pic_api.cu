@@ -124,6 +124,7 @@ const char* pic_strerror(int status)
     case PIC_ERR_UNSUPPORTED: return "unsupported configuration";
     case PIC_ERR_WORKSPACE: return "workspace too small";
     case PIC_ERR_CUDA: return "CUDA launch or runtime failure";
+    case PIC_ERR_TOO_LARGE: return "grid has more nodes than the library's static scratch array (PIC_DEPOSIT_STATIC_MAX_NODES)";
     default: return "unknown status";
     }
 }
