@@ -214,6 +214,12 @@ int pic_push(const pic_grid_t *grid, pic_particles_t *p, int order_state,
  *   PIC_SORT.  What cannot be checked is the caller's statement itself: particle data changed in place between
  *   the two calls gives a wrong order.  In a chain the hint is the workspace's own copy of the previous
  *   offsets; cell_offsets is only written.
+ *   NOTHING ELSE MAY TOUCH THE WORKSPACE between two chained steps.  The signature that vouches for the emission is
+ *   the first 256 bytes of the workspace, for every N and grid, and every other call of this library that is given
+ *   a workspace ends the chain there (pic_sort*, pic_deposit* with a workspace, pic_field_solve, pic_step with
+ *   do_sort = 0 or PIC_SORT, pic_step_buckets, pic_step_selfconsistent): the next PIC_SORT_CHAINED call then simply
+ *   sorts like PIC_SORT.  Writes of the caller's own into the workspace are covered only as far as they hit those
+ *   first bytes; past them they corrupt the emission unseen (wrong order, possibly out-of-bounds indices).
  * do_sort = 0: particles keep their order (out_a[j] = advanced in_a[j]; out may be the same arrays as
  * in); perm is not written and cell_offsets is not modified.  cell_offsets NULL says "no order at all": the any-order
  * kernels run (threads on particles, setrho 3.3.4).  cell_offsets non-NULL says "these particles

@@ -84,6 +84,14 @@ static bool aliases(const pic_grid_t& g, const pic_particles_t& a, const pic_par
     return false;
 }
 
+// A call that uses a workspace for anything but a chained step ends the chain a previous pic_step may have left in
+// it (PIC_SORT_CHAINED): the signature sits in the first bytes of every workspace layout, whatever n and the grid are.
+static int void_chain(void* ws, cudaStream_t st)
+{
+    static_assert(sizeof(ChainSig) <= 256, "the signature has the first 256 bytes of the workspace");
+    return cudaMemsetAsync(ws, 0, sizeof(ChainSig), st) == cudaSuccess ? PIC_OK : PIC_ERR_CUDA;
+}
+
 static int check_bucket(const pic_grid_t& g, const int32_t* bucket)
 {
     if (!bucket) return PIC_ERR_INVALID_ARG;
@@ -172,6 +180,7 @@ int pic_deposit(const pic_grid_t* grid, const pic_particles_t* p, int order_stat
     if (order_state < PIC_ORDER_UNSORTED || order_state > PIC_ORDER_STALE) return PIC_ERR_INVALID_ARG;
     if (order_state != PIC_ORDER_UNSORTED && !aligned16(cell_offsets)) return PIC_ERR_INVALID_ARG;
     if (!aligned16(rho)) return PIC_ERR_INVALID_ARG;
+    if (racc && (rc = void_chain(ws, (cudaStream_t)stream)) != PIC_OK) return rc;     // the workspace is written: no chain from here
     mark_phase(PIC_PHASE_BEGIN, (cudaStream_t)stream);
     rc = launch_deposit(*grid, *p, order_state, cell_offsets, rho, racc, (cudaStream_t)stream);
     mark_phase(PIC_PHASE_DEPOSIT, (cudaStream_t)stream);
@@ -188,6 +197,7 @@ int pic_deposit_nodes(const pic_grid_t* grid, const pic_particles_t* p, const in
     if (!aligned16(cell_offsets) || !aligned16(rho) || !aligned16(ws)) return PIC_ERR_INVALID_ARG;
     SortWs sws;
     if ((rc = carve_sort_ws(*grid, p->n, ws, ws_bytes, sws)) != PIC_OK) return rc;
+    if ((rc = void_chain(ws, (cudaStream_t)stream)) != PIC_OK) return rc;
     mark_phase(PIC_PHASE_BEGIN, (cudaStream_t)stream);
     rc = launch_deposit_nodes(*grid, *p, cell_offsets, rho, sws, (cudaStream_t)stream);
     mark_phase(PIC_PHASE_DEPOSIT, (cudaStream_t)stream);
@@ -215,6 +225,7 @@ int pic_deposit_replicated(const pic_grid_t* grid, const pic_particles_t* p, con
     if (ws_bytes < sb + replicated_slab_bytes(*grid)) return PIC_ERR_WORKSPACE;
     SortWs sws;
     if ((rc = carve_sort_ws(*grid, p->n, ws, sb, sws)) != PIC_OK) return rc;
+    if ((rc = void_chain(ws, (cudaStream_t)stream)) != PIC_OK) return rc;
     mark_phase(PIC_PHASE_BEGIN, (cudaStream_t)stream);
     rc = launch_deposit_replicated(*grid, *p, cell_offsets, rho, sws, (char*)ws + sb, (cudaStream_t)stream);
     mark_phase(PIC_PHASE_DEPOSIT, (cudaStream_t)stream);

@@ -839,7 +839,11 @@ static SortLayout sort_layout(const pic_grid_t& g, int64_t n)
     L.scan_tiles = (C + kScanTile - 1) / kScanTile;
     L.cls_tiles = (n + kClsTile - 1) / kClsTile;
     L.stage_tiles = (n + kStageTile - 1) / kStageTile;
+    // The chain signature comes FIRST, at an offset that does not depend on n or the grid: whatever else is done with
+    // this workspace -- a carve for another particle count, the field solve's arrays, a caller's own data -- lands on
+    // it (or is one of this library's calls, which void it) before it can reach the emission the signature vouches for.
     size_t off = 0;
+    L.chain_sig = off; off += 256;
     const size_t nb = align256(sizeof(uint32_t) * (size_t)(n > 0 ? n : 1));
     const size_t wb = align256(sizeof(uint32_t) * (size_t)((n + 31) / 32 + 2));
     const size_t cb = align256(sizeof(int32_t) * (size_t)(C + 1));
@@ -873,7 +877,6 @@ static SortLayout sort_layout(const pic_grid_t& g, int64_t n)
     L.cls_status = off; off += align256(sizeof(uint32_t) * (size_t)((L.stage_tiles + kScanTile - 1) / kScanTile + 1));
     L.counters = off; off += 256;
     L.zero_end = off;
-    L.chain_sig = off; off += 256;
     L.racc = off; off += align256(sizeof(double) * (size_t)C);
     L.total = off;
     return L;

@@ -647,6 +647,53 @@ def test_chain_flag_on_foreign_arrays_falls_back():
     assert np.array_equal(st.perm[:n].cpu().numpy(), ref2["perm"])
 
 
+@pytest.mark.parametrize("foreign", ["field_solve", "deposit_other_n", "deposit_nodes_other_n", "replicated_other_n"])
+def test_chain_ends_when_the_workspace_is_used_for_something_else(foreign):
+    """Between two chained steps another call is given the same workspace and writes over the emission (the field
+    solve's arrays start at the front; a deposit carved for another particle count puts its double grid in the middle
+    of the staged keys).  Each of these calls voids the chain signature in the first bytes of the workspace, so the
+    next PIC_SORT_CHAINED step must sort from the positions and still give the oracle's perm and offsets."""
+    O, B = _mods()
+    cfg = _cfg("cfg3", dict(N=40_000, n=(32, 32, 32)))          # field arrays (32 C bytes) cover keys, idx and pkey of N
+    wl = W.make_workload(cfg)
+    go, g = O.grid_of(cfg), B.grid_of(cfg)
+    n = cfg.N
+    big = torch.empty(max(B.pic_workspace_bytes(g, n), B.pic_field_solve_bytes(g), B.pic_deposit_replicated_bytes(g, 1000)) + 4096,
+                      dtype=torch.uint8, device="cuda")
+    st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E)
+    st.ws = big
+    st.step(cfg.dt, cfg.qm, True)
+    st.step(cfg.dt, cfg.qm, True)                              # chained; leaves an emission for the third step
+    torch.cuda.synchronize()
+    small = W.make_workload(cfg.scaled(1000, seed=3))
+    xs, ws_ = to_dev(small.x), to_dev([small.w])[0]
+    rho = torch.empty(g.cells, dtype=torch.float32, device="cuda")
+    if foreign == "field_solve":
+        rho.copy_(st.rho)
+        B.pic_field_solve(g, rho, [torch.empty_like(rho) for _ in range(3)], None, big)
+    elif foreign == "deposit_other_n":
+        B.pic_deposit(g, xs, ws_, rho, B.PIC_ORDER_UNSORTED, None, big)
+    else:
+        sx, _, sw, _, off = O.sort(go, small.x, small.v, small.w)
+        offd = torch.from_numpy(np.concatenate([off, np.zeros(3, np.int32)]).astype(np.int32)).cuda()
+        dep = B.pic_deposit_nodes if foreign == "deposit_nodes_other_n" else B.pic_deposit_replicated
+        dep(g, to_dev(sx), to_dev([sw])[0], rho, offd, big)
+    torch.cuda.synchronize()
+    ref = O.step(go, to_host(st.cur["x"]), to_host(st.cur["v"]), st.cur["w"].cpu().numpy(), wl.E, cfg.dt, cfg.qm)
+    st.step(cfg.dt, cfg.qm, True)                              # asks for PIC_SORT_CHAINED
+    torch.cuda.synchronize()
+    assert np.array_equal(st.cell_offsets[: g.cells + 1].cpu().numpy(), ref["cell_offsets"])
+    assert np.array_equal(st.perm[:n].cpu().numpy(), ref["perm"])
+    assert err_rho(st.rho.cpu().numpy(), ref["rho"]) <= TOL_RHO[cfg.dtype]
+    for c in range(cfg.dim):
+        assert err_x(st.cur["x"][c].cpu().numpy(), ref["x"][c], cfg.L[c]) <= TOL_XV[cfg.dtype]
+    # and the chain picks up again afterwards: one more chained step, still the oracle's order
+    ref2 = O.step(go, to_host(st.cur["x"]), to_host(st.cur["v"]), st.cur["w"].cpu().numpy(), wl.E, cfg.dt, cfg.qm)
+    st.step(cfg.dt, cfg.qm, True)
+    torch.cuda.synchronize()
+    assert np.array_equal(st.perm[:n].cpu().numpy(), ref2["perm"])
+
+
 @pytest.mark.parametrize("name,kw,mode", [("cfg1", dict(), "plain"), ("cfg3", dict(N=200_000, n=(32, 32, 32)), "plain"),
                                           ("cfg5", dict(N=8 * 16 ** 3, n=(16, 16, 16)), "closed"),
                                           ("cfg2", dict(N=100_000, n=(32, 32)), "bucket")])
