@@ -203,8 +203,8 @@ int pic_push(const pic_grid_t *grid, pic_particles_t *p, int order_state,
  * accel -> push, the paper's loop order setrho -> accel -> push with the
  * field solve left out as in the paper and the re-sort of PAPER.md:100 placed first (R6).
  * out receives the particles in sorted order, advanced to t+1; rho is the density at t.
- * do_sort = PIC_SORT (1): sort by the keys of the positions in `in`; cell_offsets is read on entry as a hint and
- *   overwritten, exactly as in pic_sort; `out` must not overlap `in`.
+ * do_sort = PIC_SORT (1), or any other non-zero value except PIC_SORT_CHAINED: sort by the keys of the positions in
+ *   `in`; cell_offsets is read on entry as a hint and overwritten, exactly as in pic_sort; `out` must not overlap `in`.
  * do_sort = PIC_SORT_CHAINED (3): the same result, for a time loop.  The caller states that `in` is, UNMODIFIED,
  *   the `out` of the previous pic_step(do_sort != 0) call made with this workspace.  That call's step kernel had
  *   every advanced position in registers and left the next keys, their histogram and the list of particles that
@@ -295,7 +295,8 @@ int pic_step_buckets(const pic_grid_t *grid, const int32_t bucket[3] /* host */,
  *
  * pic_field_solve: rho[C] -> E[c][C] for c < dim and, if phi != NULL, phi[C]; all of the grid's dtype, x fastest; the
  *   arithmetic is double whatever the dtype.  Hand-written transforms (radix-2 for power-of-two n[c], the plain DFT sum
- *   otherwise); n[c] <= 4096 else PIC_ERR_UNSUPPORTED.  ws: pic_field_solve_bytes().
+ *   otherwise); n[c] <= 4096, else PIC_ERR_UNSUPPORTED from every call of this group (the *_bytes ones included),
+ *   returned before anything is enqueued or written.  ws: pic_field_solve_bytes().
  * pic_step_selfconsistent: one step of the closed loop i-iv: sort by cell (cell_offsets: in/out hint as in
  *   pic_sort), rho = deposit at x(t) (the reorder happens in the same pass), E = field_solve(rho) written to the
  *   caller's E[c], then v += qm dt E(x), x += dt v on the sorted particles.  out, perm, cell_offsets, rho as in pic_step.

@@ -255,7 +255,8 @@ int pic_step(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
     g_launches = 0;
     int rc = check_grid(grid);
     if (rc != PIC_OK) return rc;
-    if (do_sort != 0 && do_sort != PIC_SORT && do_sort != PIC_SORT_CHAINED) return PIC_ERR_INVALID_ARG;
+    // any non-zero value asks for a sort (the ABI of SURVEY 8(b)); PIC_SORT_CHAINED alone asks for the chained one
+    const bool chained = do_sort == PIC_SORT_CHAINED;
     if ((rc = check_particles(*grid, in, true, true)) != PIC_OK) return rc;
     if ((rc = check_particles(*grid, out, true, true, in->n)) != PIC_OK) return rc;
     if ((rc = check_field(*grid, E)) != PIC_OK) return rc;
@@ -267,11 +268,16 @@ int pic_step(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
     if (!aligned16(ws)) return PIC_ERR_INVALID_ARG;
     SortWs sws;
     if ((rc = carve_sort_ws(*grid, in->n, ws, ws_bytes, sws)) != PIC_OK) return rc;
+    // every argument is checked before the first copy or launch is enqueued
     if (do_sort) {
         if ((in->n > 0 && !aligned16(perm)) || !aligned16(cell_offsets)) return PIC_ERR_INVALID_ARG;
         if (in->n > 0 && aliases(*grid, *in, *out, in->n)) return PIC_ERR_INVALID_ARG;
+    } else if (cell_offsets && in->n > 0 && !aligned16(cell_offsets)) {
+        return PIC_ERR_INVALID_ARG;
+    }
+    if (do_sort) {
         // perm and cell_offsets only: the reorder itself happens inside the fused kernel below
-        if ((rc = launch_sort(*grid, *in, o, perm, cell_offsets, sws, false, (do_sort & PIC_SORT_CHAINED) == PIC_SORT_CHAINED, st)) != PIC_OK) return rc;
+        if ((rc = launch_sort(*grid, *in, o, perm, cell_offsets, sws, false, chained, st)) != PIC_OK) return rc;
     } else {
         // keep the current order; out may be the same arrays as in (in-place step)
         for (int c = 0; c < grid->dim; ++c) {
@@ -289,7 +295,6 @@ int pic_step(const pic_grid_t* grid, const pic_particles_t* in, pic_particles_t*
     if (cell_offsets && in->n > 0) {
         // the order of an earlier sort: the same kernel in place.  It finds the runs of equal cell key itself
         // (cell_offsets is not read), so the result is exact however far the particles have drifted
-        if (!aligned16(cell_offsets)) return PIC_ERR_INVALID_ARG;
         rc = launch_fused(*grid, o, o, nullptr, sws, rho, E, dt, qm, st);
         mark_phase(PIC_PHASE_PUSH, st);
         return rc;
@@ -393,6 +398,7 @@ int pic_field_solve_bytes(const pic_grid_t* grid, size_t* bytes)
     int rc = check_grid(grid);
     if (rc != PIC_OK) return rc;
     if (!bytes) return PIC_ERR_INVALID_ARG;
+    if ((rc = field_supported(*grid)) != PIC_OK) return rc;
     *bytes = field_ws_bytes(*grid);
     return PIC_OK;
 }
@@ -405,6 +411,7 @@ int pic_field_solve(const pic_grid_t* grid, const void* rho, void* const E[3], v
     if (!aligned16(rho) || !E || !aligned16(ws) || (phi && !aligned16(phi))) return PIC_ERR_INVALID_ARG;
     for (int c = 0; c < grid->dim; ++c)
         if (!aligned16(E[c])) return PIC_ERR_INVALID_ARG;
+    if ((rc = field_supported(*grid)) != PIC_OK) return rc;          // before anything is enqueued
     if (ws_bytes < field_ws_bytes(*grid)) return PIC_ERR_WORKSPACE;
     return launch_field_solve(*grid, rho, E, phi, ws, (cudaStream_t)stream);
 }
@@ -414,6 +421,7 @@ int pic_step_selfconsistent_bytes(const pic_grid_t* grid, int64_t n, size_t* byt
     int rc = check_grid(grid);
     if (rc != PIC_OK) return rc;
     if (!bytes || n < 0 || n >= ((int64_t)1 << 30)) return PIC_ERR_INVALID_ARG;
+    if ((rc = field_supported(*grid)) != PIC_OK) return rc;
     *bytes = sort_ws_bytes(*grid, n) + field_ws_bytes(*grid);
     return PIC_OK;
 }
@@ -432,6 +440,7 @@ int pic_step_selfconsistent(const pic_grid_t* grid, const pic_particles_t* in, p
         if (!aligned16(E[c])) return PIC_ERR_INVALID_ARG;
     if ((in->n > 0 && !aligned16(perm)) || !aligned16(cell_offsets)) return PIC_ERR_INVALID_ARG;
     if (in->n > 0 && aliases(*grid, *in, *out, in->n)) return PIC_ERR_INVALID_ARG;
+    if ((rc = field_supported(*grid)) != PIC_OK) return rc;          // before the sort and the deposit are enqueued
     const size_t sb = sort_ws_bytes(*grid, in->n);
     if (ws_bytes < sb + field_ws_bytes(*grid)) return PIC_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;

@@ -286,6 +286,9 @@ int launch_deposit_nodes(const pic_grid_t& g, const pic_particles_t& p, const in
                          const SortWs& ws, cudaStream_t st);
 // periodic Poisson solve (pic_field.cu): rho -> E[c] (and phi if not NULL), all [C] of the grid's dtype; ws: field_ws_bytes
 size_t field_ws_bytes(const pic_grid_t& g);
+// PIC_OK, or PIC_ERR_UNSUPPORTED if an axis is longer than this build's transforms take (n[c] <= 4096): checked by the
+// entry points before anything is enqueued
+int field_supported(const pic_grid_t& g);
 int launch_field_solve(const pic_grid_t& g, const void* rho, void* const E[3], void* phi, void* ws, cudaStream_t st);
 // the closed loop i-iv: deposit along perm (+ reorder into p), field solve, gather + accel + push in place
 int launch_selfconsistent(const pic_grid_t& g, const pic_particles_t& src, pic_particles_t& p, const int32_t* perm,

@@ -144,13 +144,40 @@ size_t field_ws_bytes(const pic_grid_t& g)
 }
 
 // lines per block and dynamic shared memory for an axis of length n (0: too long for this build)
+constexpr size_t kFieldSmemBudget = 200 * 1024;
+constexpr int kFieldMaxN = 4096;          // the bound pic.h documents (the shared-memory budget alone would allow 4266)
 static int lines_per_block(int n, size_t& smem)
 {
-    const size_t budget = 200 * 1024;
+    const size_t budget = kFieldSmemBudget;
+    if (n > kFieldMaxN) { smem = 0; return 0; }
     int lb = 8;
     while (lb > 1 && sizeof(cplx) * ((size_t)2 * lb * n + n) > 64 * 1024) lb >>= 1;
     smem = sizeof(cplx) * ((size_t)2 * lb * n + n);
     return smem <= budget ? lb : 0;
+}
+
+// PIC_OK if every axis has a transform in this build, else PIC_ERR_UNSUPPORTED: asked BEFORE anything is enqueued
+int field_supported(const pic_grid_t& g)
+{
+    for (int c = 0; c < g.dim; ++c) {
+        size_t smem = 0;
+        if (lines_per_block(g.n[c], smem) == 0) return PIC_ERR_UNSUPPORTED;
+    }
+    return PIC_OK;
+}
+
+// The transforms of long axes need more dynamic shared memory than the default limit: raised to the budget once per
+// device and kernel, not on every call.
+template <bool POW2>
+static int raise_smem_limit_once()
+{
+    static bool done[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return PIC_ERR_CUDA;
+    if (dev >= 0 && dev < 64 && done[dev]) return PIC_OK;
+    PIC_CUDA_OK(cudaFuncSetAttribute(k_fft_axis<POW2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFieldSmemBudget));
+    if (dev >= 0 && dev < 64) done[dev] = true;
+    return PIC_OK;
 }
 
 static int fft_all_axes(const pic_grid_t& g, cplx* data, double sign, cudaStream_t st)
@@ -167,7 +194,10 @@ static int fft_all_axes(const pic_grid_t& g, cplx* data, double sign, cudaStream
         const unsigned blocks = (unsigned)((nlines + lb - 1) / lb);
         const bool pow2 = (n & (n - 1)) == 0;
         auto kern = pow2 ? k_fft_axis<true> : k_fft_axis<false>;
-        if (smem > 48 * 1024) PIC_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (smem > 48 * 1024) {
+            const int rc = pow2 ? raise_smem_limit_once<true>() : raise_smem_limit_once<false>();
+            if (rc != PIC_OK) return rc;
+        }
         kern<<<blocks, 256, smem, st>>>(data, n, inner, nlines, lb, sign);
         count_launch();
         inner *= n;

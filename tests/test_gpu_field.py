@@ -75,9 +75,33 @@ def test_field_solve_rejects_what_it_cannot_do():
     g = B.Grid(2, (8192, 4), (1.0, 1.0), 1, "f64")
     rho = torch.zeros(g.cells, dtype=torch.float64, device="cuda")
     E = [torch.zeros_like(rho), torch.zeros_like(rho)]
-    ws = torch.empty(B.pic_field_solve_bytes(g), dtype=torch.uint8, device="cuda")
+    ws = torch.empty(2 * 16 * g.cells + 1024, dtype=torch.uint8, device="cuda")
+    for call in (lambda: B.pic_field_solve_bytes(g), lambda: B.pic_step_selfconsistent_bytes(g, 10),
+                 lambda: B.pic_field_solve(g, rho, E, None, ws)):
+        with pytest.raises(B.PicError, match="unsupported"):
+            call()
+    # the documented bound is the enforced one: 4096 is taken, 4097 is not (the check comes before any launch)
+    B.pic_field_solve_bytes(B.Grid(2, (4096, 4), (1.0, 1.0), 1, "f64"))
     with pytest.raises(B.PicError, match="unsupported"):
-        B.pic_field_solve(g, rho, E, None, ws)
+        B.pic_field_solve_bytes(B.Grid(2, (4, 4097), (1.0, 1.0), 1, "f64"))
+    # the closed loop refuses BEFORE the sort and the deposit: out, perm and rho keep what they held
+    gc = B.Grid(2, (8192, 4), (1.0, 1.0), 1, "f64")
+    n = 64
+    x = [torch.rand(n, dtype=torch.float64, device="cuda") * 4 for _ in range(2)]
+    v = [torch.zeros(n, dtype=torch.float64, device="cuda") for _ in range(2)]
+    w = torch.ones(n, dtype=torch.float64, device="cuda")
+    xo = [torch.full((n,), -1.0, dtype=torch.float64, device="cuda") for _ in range(2)]
+    vo = [torch.full((n,), -1.0, dtype=torch.float64, device="cuda") for _ in range(2)]
+    wo = torch.full((n,), -1.0, dtype=torch.float64, device="cuda")
+    perm = torch.full((n,), -5, dtype=torch.int32, device="cuda")
+    off = torch.zeros(gc.cells + 4, dtype=torch.int32, device="cuda")
+    rho_c = torch.full((gc.cells,), -2.0, dtype=torch.float64, device="cuda")
+    Ec = [torch.zeros(gc.cells, dtype=torch.float64, device="cuda") for _ in range(2)]
+    wsc = torch.empty(B.pic_workspace_bytes(gc, n) + 2 * 16 * gc.cells + 1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.PicError, match="unsupported"):
+        B.pic_step_selfconsistent(gc, x, v, w, xo, vo, wo, perm, off, rho_c, Ec, 0.1, 1.0, wsc)
+    torch.cuda.synchronize()
+    assert torch.all(perm == -5).item() and torch.all(rho_c == -2.0).item() and torch.all(wo == -1.0).item()
     g2 = B.Grid(2, (16, 16), (1.0, 1.0), 1, "f64")
     with pytest.raises(B.PicError, match="workspace"):
         B.pic_field_solve(g2, rho[:256], [E[0][:256], E[1][:256]], None, ws[:64])

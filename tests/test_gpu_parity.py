@@ -647,6 +647,36 @@ def test_chain_flag_on_foreign_arrays_falls_back():
     assert np.array_equal(st.perm[:n].cpu().numpy(), ref2["perm"])
 
 
+def test_pic_step_do_sort_values_and_checks_before_any_copy():
+    """any non-zero do_sort sorts (only PIC_SORT_CHAINED means more); and a bad argument is reported before
+    anything is enqueued -- with do_sort = 0 and distinct out arrays that includes the device-to-device copies."""
+    O, B = _mods()
+    cfg = _cfg("cfg3", dict(N=30_001, n=(16, 16, 16)))
+    wl = W.make_workload(cfg)
+    go, g = O.grid_of(cfg), B.grid_of(cfg)
+    n = cfg.N
+    ref = O.step(go, wl.x, wl.v, wl.w, wl.E, cfg.dt, cfg.qm)
+    x, v, w, E = to_dev(wl.x), to_dev(wl.v), to_dev([wl.w])[0], to_dev(wl.E)
+    ws = torch.empty(B.pic_workspace_bytes(g, n), dtype=torch.uint8, device="cuda")
+    rho = torch.empty(g.cells, dtype=g.torch_dtype, device="cuda")
+    for do_sort in (2, 7, -1, True):
+        xo, vo, wo = [torch.empty_like(a) for a in x], [torch.empty_like(a) for a in v], torch.empty_like(w)
+        perm = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+        off = torch.zeros(g.cells + 4, dtype=torch.int32, device="cuda")
+        B.pic_step(g, x, v, w, xo, vo, wo, perm, off, rho, E, cfg.dt, cfg.qm, do_sort, ws)
+        torch.cuda.synchronize()
+        assert np.array_equal(perm.cpu().numpy(), ref["perm"]), do_sort
+        assert np.array_equal(off[: g.cells + 1].cpu().numpy(), ref["cell_offsets"]), do_sort
+        assert err_x(xo[0].cpu().numpy(), ref["x"][0], cfg.L[0]) <= TOL_XV[cfg.dtype]
+    # do_sort = 0 with a misaligned cell_offsets: refused, and `out` has not been written
+    xo, vo, wo = [torch.full_like(a, -1.0) for a in x], [torch.full_like(a, -1.0) for a in v], torch.full_like(w, -1.0)
+    off = torch.zeros(g.cells + 8, dtype=torch.int32, device="cuda")
+    with pytest.raises(B.PicError, match="invalid argument"):
+        B.pic_step(g, x, v, w, xo, vo, wo, None, off[1:], rho, E, cfg.dt, cfg.qm, 0, ws)
+    torch.cuda.synchronize()
+    assert all(torch.all(a == -1.0).item() for a in xo + vo + [wo])
+
+
 @pytest.mark.parametrize("foreign", ["field_solve", "deposit_other_n", "deposit_nodes_other_n", "replicated_other_n"])
 def test_chain_ends_when_the_workspace_is_used_for_something_else(foreign):
     """Between two chained steps another call is given the same workspace and writes over the emission (the field
