@@ -11,9 +11,14 @@ void count_launch(int n) { g_launches += n; }
 
 int sm_count()
 {
+    // asked several times per step: the attribute query is made once per device (a benign race: every thread that
+    // loses it writes the same number)
+    static int cached[64] = {};
     int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-        return 148;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+    if (dev >= 0 && dev < 64 && cached[dev] > 0) return cached[dev];
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) return 148;
+    if (dev >= 0 && dev < 64) cached[dev] = sms;
     return sms;
 }
 

@@ -243,7 +243,7 @@ struct SortWs {
     int32_t* prev_off;       // [C+1] cell_offsets as the last sort of a chain wrote them (the next one's hint)
     ChainSig* chain_sig;     // what that step worked on
     EmitP emit;              // where a step kernel leaves the next sort's inputs
-    void* hist_begin;        // cell_count, mover_count, mover_lo: zeroed before k_classify, written by k_chain_counts in a chain
+    void* hist_begin;        // cell_count, mover_count, mover_lo: zeroed before k_classify, or in a chain formed from the emitted counters (k_hint_hist)
     size_t hist_bytes;
     void* emit_begin;        // emit.cell_out, emit.mover_in: zeroed before an emitting step kernel
     size_t emit_bytes;

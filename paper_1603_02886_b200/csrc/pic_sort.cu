@@ -21,10 +21,10 @@
 //   * the full-key histogram and its exclusive scan give cell_offsets; the movers' histogram and
 //     its scan place each mover inside its cell.
 //
-// Kernels:  k_hint_check     hint -> private copy, validity flag; is this call the next link of a chain?
+// Kernels:  k_hint_hist      hint -> private copy, validity flag; is this call the next link of a chain?  The three
+//                            histograms: zero, or in a chain formed from the step kernel's per-cell in/out counters
 //           k_classify       x[d] -> key (cell or bucket), histograms, stayer/mover split, movers staged per 2048 positions
 //                            (returns at once in a chain: the previous step kernel has emitted all of it)
-//           k_chain_counts   in a chain: the three histograms from the step kernel's per-cell in/out counters
 //           k_scan_cells     count[C] -> exclusive offsets [C+1] (single pass, decoupled look-back)
 //           k_movers_place   staged movers -> one list in position order
 //           k_scan_digits    digit histograms -> exclusive global digit offsets
@@ -116,10 +116,17 @@ __device__ __forceinline__ bool chain_holds(const ChainSig* sig, const ChainSig&
 
 // private copy of the hint: cell_offsets as found on entry, or -- in a chain -- the offsets the previous step
 // wrote (kept in the workspace, so that the emitted stayer/mover split and the hint cannot disagree);
-// bad = 1 unless 0 <= h[0] <= h[1] <= ... <= h[C] <= N
-__global__ void __launch_bounds__(256) k_hint_check(const int32_t* __restrict__ hint, const int32_t* __restrict__ prev_off,
-                                                    const ChainSig* __restrict__ sig, ChainSig want, int chain_req,
-                                                    int32_t* __restrict__ old_off, int C, int64_t n, uint32_t* counters)
+// bad = 1 unless 0 <= h[0] <= h[1] <= ... <= h[C] <= N.
+// The same threads prepare the three histograms (one launch instead of three: small problems are launch bound).  Not a
+// chain: they are zero before k_classify fills them.  A chain: they come from what the previous step kernel counted --
+// particles that left each cell, movers into it, and how many of those come from below: count = old count - out + in.
+// Every block decides "chain or not" for itself from the signature, so there is no dependence between blocks.
+__global__ void __launch_bounds__(256) k_hint_hist(const int32_t* __restrict__ hint, const int32_t* __restrict__ prev_off,
+                                                   const ChainSig* __restrict__ sig, ChainSig want, int chain_req,
+                                                   int32_t* __restrict__ old_off, int C, int64_t n, uint32_t* counters,
+                                                   const int32_t* __restrict__ cell_out, const unsigned long long* __restrict__ mover_in,
+                                                   int32_t* __restrict__ cell_count, int32_t* __restrict__ mover_count,
+                                                   int32_t* __restrict__ mover_lo)
 {
     __shared__ int s_chain;
     if (threadIdx.x == 0) {
@@ -133,33 +140,23 @@ __global__ void __launch_bounds__(256) k_hint_check(const int32_t* __restrict__ 
     const int32_t a = h[k];
     old_off[k] = a;
     bool bad = a < 0 || (int64_t)a > n;
-    if (k < C) bad = bad || h[k + 1] < a;
+    int32_t b = a;
+    if (k < C) {
+        b = h[k + 1];
+        bad = bad || b < a;
+    }
     if (bad) counters[kCtrHintBad] = 1u;
-}
-
-// the three histograms are zero before k_classify fills them; in a chain the previous step kernel has filled them
-__global__ void __launch_bounds__(256) k_zero_hist(uint4* __restrict__ p, size_t n16, const uint32_t* __restrict__ counters)
-{
-    if (counters[kCtrChain]) return;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x)
-        p[i] = make_uint4(0u, 0u, 0u, 0u);
-}
-
-// In a chain the three histograms come from what the previous step kernel counted: particles that left each cell,
-// movers into it, and how many of those come from below.  count = old count - out + in.
-__global__ void __launch_bounds__(256) k_chain_counts(const int32_t* __restrict__ old_off, const int32_t* __restrict__ cell_out,
-                                                      const unsigned long long* __restrict__ mover_in, int32_t* __restrict__ cell_count,
-                                                      int32_t* __restrict__ mover_count, int32_t* __restrict__ mover_lo, int C,
-                                                      const uint32_t* __restrict__ counters)
-{
-    if (!counters[kCtrChain]) return;
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= C) return;
-    const unsigned long long in = mover_in[k];
-    const int32_t min = (int32_t)(uint32_t)in;
-    mover_count[k] = min;
-    mover_lo[k] = (int32_t)(uint32_t)(in >> 32);
-    cell_count[k] = old_off[k + 1] - old_off[k] - cell_out[k] + min;
+    if (!s_chain) {
+        cell_count[k] = 0;
+        mover_count[k] = 0;
+        mover_lo[k] = 0;
+    } else if (k < C) {
+        const unsigned long long in = mover_in[k];
+        const int32_t min = (int32_t)(uint32_t)in;
+        mover_count[k] = min;
+        mover_lo[k] = (int32_t)(uint32_t)(in >> 32);
+        cell_count[k] = b - a - cell_out[k] + min;
+    }
 }
 
 // the step has left its emission behind: the next call may chain on to it
@@ -988,15 +985,13 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
     mark_phase(PIC_PHASE_BEGIN, st);
     PIC_CUDA_OK(cudaMemsetAsync(ws.zero_begin, 0, ws.zero_bytes, st));
     // the hint: cell_offsets as found on entry -- or, in a chain, what the previous step left in the workspace
-    k_hint_check<<<(unsigned)((C + 1 + 255) / 256), 256, 0, st>>>(cell_offsets, ws.prev_off, ws.chain_sig, chain_sig_of(g, in),
-                                                                  chained ? 1 : 0, ws.old_off, C, n, ws.counters);
+    k_hint_hist<<<(unsigned)((C + 1 + 255) / 256), 256, 0, st>>>(cell_offsets, ws.prev_off, ws.chain_sig, chain_sig_of(g, in),
+                                                                 chained ? 1 : 0, ws.old_off, C, n, ws.counters, ws.emit.cell_out,
+                                                                 ws.emit.mover_in, ws.cell_count, ws.mover_count, ws.mover_lo);
     count_launch();
     if (n > 0) {
         // not a chain: keys, histograms and the stayer/mover split from the positions.  Movers are staged per tile in
         // the second halves of the ping-pong arrays, then packed
-        k_zero_hist<<<sm_count() * 4, 256, 0, st>>>((uint4*)ws.hist_begin, ws.hist_bytes / 16, ws.counters);
-        k_chain_counts<<<(unsigned)((C + 255) / 256), 256, 0, st>>>(ws.old_off, ws.emit.cell_out, ws.emit.mover_in, ws.cell_count,
-                                                                    ws.mover_count, ws.mover_lo, C, ws.counters);
         auto classify = ws.bucket ? k_classify<T, D, true> : k_classify<T, D, false>;
         classify<<<(unsigned)ws.cls_tiles, kClsThreads, 0, st>>>(
             make_partp<T>(in), make_gridp<T>(g, ws.bucket), (int)n, ws.old_off, ws.cell_count, ws.mover_count, ws.mover_lo, ws.keys[1],
@@ -1006,7 +1001,7 @@ static int sort_keys_perm(const pic_grid_t& g, const pic_particles_t& in, int32_
         k_movers_place<<<(unsigned)ws.stage_tiles, 256, 0, st>>>(ws.keys[1], ws.idx[1], ws.keys[0], ws.idx[0], ws.mask,
                                                                 ws.mprefix, ws.tile_base, (int)ws.stage_tiles, n, ws.counters,
                                                                 ws.chain_sig);
-        count_launch(5);
+        count_launch(3);
         if (holes) PIC_CUDA_OK(cudaMemcpyAsync(holes, ws.idx[0], sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToDevice, st));
     } else {
         PIC_CUDA_OK(cudaMemsetAsync(ws.hist_begin, 0, ws.hist_bytes, st));
