@@ -16,7 +16,7 @@
  *
  * A second, TIMED-ONLY build (oracle.build_openmp(): the same file with -fopenmp,
  * libpicref_omp.so) spreads the particle loops of the key pass, the attribute move,
- * the deposit (one private grid per thread, added up at the end) and the push over
+ * the deposit (one private grid per thread, added up node by node at the end) and the push over
  * the host cores: it mirrors the paper's own CPU reference, OpenMP on 8 cores
  * (PAPER.md:388), for bench.py's cpu_baseline.  Everything between `#ifdef _OPENMP`
  * belongs to that build; the parity tests load the plain build only, whose
@@ -37,6 +37,9 @@
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+#ifdef _OPENMP
+#include <omp.h>                                         /* timed OpenMP build only, see the header */
+#endif
 
 typedef struct {
     int32_t dim;      /* 2 or 3 */
@@ -210,8 +213,11 @@ int pic_ref_sort(const pic_ref_grid *g, int64_t n,
     for (int64_t k = 0; k <= C; ++k) cell_offsets[k] = 0;
 #ifdef _OPENMP                                           /* timed OpenMP build only, see the header */
 #pragma omp parallel for schedule(static)
-    for (int64_t i = 0; i < n; ++i) key[i] = cell_key(g, xin, i);
-    for (int64_t i = 0; i < n; ++i) cell_offsets[key[i] + 1] += 1;
+    for (int64_t i = 0; i < n; ++i) {
+        key[i] = cell_key(g, xin, i);
+#pragma omp atomic
+        cell_offsets[key[i] + 1] += 1;
+    }
 #else
     for (int64_t i = 0; i < n; ++i) {                    /* histogram */
         key[i] = cell_key(g, xin, i);
@@ -428,15 +434,34 @@ int pic_ref_deposit(const pic_ref_grid *g, int64_t n, const void *const x[3], co
 #ifdef _OPENMP
     /* Timed OpenMP build only (see the header): particles split over the threads, one private grid per
      * thread, the grids added up at the end.  The summation order differs from the plain build. */
+    int max_threads = omp_get_max_threads(), bad = 0;
+    double **priv = (double **)calloc((size_t)max_threads, sizeof(double *));
+    if (!priv) return REF_BAD_ARG;
 #pragma omp parallel
     {
-        double *priv = (double *)calloc((size_t)C, sizeof(double));
+        int t = omp_get_thread_num(), nt = omp_get_num_threads();
+        priv[t] = (double *)calloc((size_t)C, sizeof(double));
+        if (!priv[t]) {
+#pragma omp atomic write
+            bad = 1;
+        }
+#pragma omp barrier
+        if (!bad) {
 #pragma omp for schedule(static)
-        for (int64_t i = 0; i < n; ++i) deposit_one(g, x, w, i, inv_vol, priv);
-#pragma omp critical
-        for (int64_t k = 0; k < C; ++k) rho[k] += priv[k];
-        free(priv);
+            for (int64_t i = 0; i < n; ++i) deposit_one(g, x, w, i, inv_vol, priv[t]);
+            /* the grids are added up node by node, threads in ascending order: parallel over the nodes, no critical
+             * section */
+#pragma omp for schedule(static)
+            for (int64_t k = 0; k < C; ++k) {
+                double sum = 0.0;
+                for (int u = 0; u < nt; ++u) sum += priv[u][k];
+                rho[k] = sum;
+            }
+        }
     }
+    for (int u = 0; u < max_threads; ++u) free(priv[u]);
+    free(priv);
+    if (bad) return REF_BAD_ARG;
 #else
     for (int64_t i = 0; i < n; ++i) deposit_one(g, x, w, i, inv_vol, rho);
 #endif
