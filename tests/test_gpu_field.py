@@ -137,11 +137,17 @@ def test_closed_loop_lockstep(name, N, kw):
         assert np.array_equal(off[: gb.cells + 1].cpu().numpy(), ref["cell_offsets"])
         assert err_rho(rho.cpu().numpy(), ref["rho"]) <= TOL_RHO[cfg.dtype]
         emax = max(np.max(np.abs(e.astype(np.float64))) for e in ref["E"])
-        for c in range(cfg.dim):
-            # E inherits the deposit's rounding (rho is stored in the grid dtype before the solve)
-            assert np.max(np.abs(E[c].cpu().numpy().astype(np.float64) - ref["E"][c].astype(np.float64))) <= 10 * TOL_RHO[cfg.dtype] * emax
-            assert err_x(xo[c].cpu().numpy(), ref["x"][c], cfg.L[c]) <= 10 * TOL_XV[cfg.dtype], "x at step %d" % k
-            assert err_v(vo[c].cpu().numpy(), ref["v"][c]) <= 10 * TOL_XV[cfg.dtype], "v at step %d" % k
+        # E inherits the deposit's rounding (rho is stored in the grid dtype before the solve), x and v inherit E's; all
+        # stay within the STATED tolerances (achieved on B200, round 3: E 8e-15 / 3.2e-7, x 2.2e-16 / 9.5e-8, v 2e-16 /
+        # 1.7e-7 in fp64 / fp32; the bounds were 10 x the tolerances before).  Printed: pytest -s or -rP shows them
+        eE = max(np.max(np.abs(E[c].cpu().numpy().astype(np.float64) - ref["E"][c].astype(np.float64))) for c in range(cfg.dim)) / emax
+        ex = max(err_x(xo[c].cpu().numpy(), ref["x"][c], cfg.L[c]) for c in range(cfg.dim))
+        ev = max(err_v(vo[c].cpu().numpy(), ref["v"][c]) for c in range(cfg.dim))
+        print("closed loop %s step %d: achieved E %.3g (bound %.0e), x %.3g, v %.3g (bound %.0e)"
+              % (name, k, eE, TOL_RHO[cfg.dtype], ex, ev, TOL_XV[cfg.dtype]))
+        assert eE <= TOL_RHO[cfg.dtype]
+        assert ex <= TOL_XV[cfg.dtype], "x at step %d" % k
+        assert ev <= TOL_XV[cfg.dtype], "v at step %d" % k
         x, v, w = ref["x"], ref["v"], ref["w"]
 
 

@@ -77,20 +77,22 @@ def test_full_size_elementwise(name):
 
 
 @pytest.mark.timeout(1200)
-@pytest.mark.parametrize("name", ["cfg2", "cfg5_8"])
+@pytest.mark.parametrize("name", ["cfg2", "cfg5_8", "cfg5_512"])
 def test_full_size_elementwise_fp64(name):
     """The fp64 configs at full size, every element, one step from the seeded order and one from the GPU's state:
-    cfg2 (1e7 particles) and cfg5 at 8 particles per cell (2.1e6)."""
+    cfg2 (1e7 particles) and cfg5 at 8 particles per cell (2.1e6); cfg5 at 512 per cell (1.34e8 particles, the largest
+    configuration of BASELINE.json; sort every step) for ONE step from the seeded order -- the oracle needs about a
+    minute for it."""
     import oracle as O
     import paper_1603_02886_b200 as B
 
-    cfg = W.cfg5(8, 1) if name == "cfg5_8" else W.CONFIGS[name]
+    cfg = W.cfg5(512, 1) if name == "cfg5_512" else (W.cfg5(8, 1) if name == "cfg5_8" else W.CONFIGS[name])
     n, d = cfg.N, cfg.dim
     wl = W.make_workload(cfg)
     g, go = B.grid_of(cfg), O.grid_of(cfg)
     st = B.Stepper(g, wl.x, wl.v, wl.w, wl.E, device="cuda:0")
     x, v, w = wl.x, wl.v, wl.w
-    for step in range(2):
+    for step in range(1 if name == "cfg5_512" else 2):
         ref = O.step(go, x, v, w, wl.E, cfg.dt, cfg.qm)
         st.step(cfg.dt, cfg.qm, True)
         torch.cuda.synchronize()
@@ -104,6 +106,10 @@ def test_full_size_elementwise_fp64(name):
             assert err_v(out["v"][c], ref["v"][c]) <= TOL_XV[cfg.dtype]
         assert np.array_equal(out["w"], ref["w"])
         x, v, w = out["x"], out["v"], out["w"]
+        del ref, rho
+    del st, wl, out, x, v, w
+    gc.collect()
+    torch.cuda.empty_cache()
 
 
 @pytest.mark.timeout(1200)

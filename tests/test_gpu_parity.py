@@ -298,11 +298,15 @@ def test_step_free_running_by_particle_id(name, kw):
     inv_g[ig] = np.arange(cfg.N)
     inv_r[ident_r] = np.arange(cfg.N)
     # a 1-ulp difference can move a particle across a cell face and change later perms; x and v by id must still agree
-    for c in range(cfg.dim):
-        xg = st.cur["x"][c].cpu().numpy()[inv_g]
-        vg = st.cur["v"][c].cpu().numpy()[inv_g]
-        assert err_x(xg, x[c][inv_r], cfg.L[c]) <= 10 * TOL_XV[cfg.dtype]
-        assert err_v(vg, v[c][inv_r]) <= 10 * TOL_XV[cfg.dtype]
+    # (ten free-running steps: still within the stated one-step tolerance -- achieved on B200 2.2e-16 / 2.8e-16 in
+    # fp64 and 1.8e-7 / 1.5e-7 in fp32 (round 3; it was 10 x the tolerance before).  The achieved error is printed:
+    # pytest -s or -rP shows it)
+    ex = max(err_x(st.cur["x"][c].cpu().numpy()[inv_g], x[c][inv_r], cfg.L[c]) for c in range(cfg.dim))
+    ev = max(err_v(st.cur["v"][c].cpu().numpy()[inv_g], v[c][inv_r]) for c in range(cfg.dim))
+    print("free-running %s: achieved err_x %.3g, err_v %.3g; tolerance %.0e"
+          % (name, ex, ev, TOL_XV[cfg.dtype]))
+    assert ex <= TOL_XV[cfg.dtype]
+    assert ev <= TOL_XV[cfg.dtype]
     mism = int(np.sum(ig != ident_r))
     assert mism <= (0 if cfg.dtype == "f64" else cfg.N // 1000), "order mismatches: %d" % mism
 
